@@ -1,0 +1,250 @@
+"""Pins for the fp64 CPU oracle (oracle/oracle.c and oracle/oracle_np.py) -- CPU only.
+
+The paper prints no worked numbers, so the oracle is pinned by closed forms (tests/golden/closed_forms.json,
+derived by hand from eq. (9)-(11)), invariants, limits and brute force, chosen so that a
+dropped term, a wrong sign/power/index or a transposed operand fails at least one of them (SURVEY.md 8(c),
+pins P1-P10).
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle, oracle_np
+from paper_1205_1222_b200 import inputs
+
+GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "closed_forms.json")))
+
+
+def _plummer(n, seed_sub=3):
+    rngs = inputs.streams(6, seed_sub)
+    x, v = inputs.plummer_points(rngs, n)
+    m = inputs.salpeter_masses(rngs["mass"], n)  # unequal masses: catches m_i / m_j mix-ups
+    return x, v, m
+
+
+def _rel(a, b):
+    return np.linalg.norm(a - b, axis=-1) / np.linalg.norm(b, axis=-1)
+
+
+# ---------------------------------------------------------------- P1 two-body closed form
+@pytest.mark.parametrize("impl", [oracle, oracle_np])
+def test_p1_two_body(impl):
+    g = GOLD["P1_two_body"]
+    xp = np.array([g["xi"], g["xj"]], dtype=float)
+    vp = np.array([g["vi"], g["vj"]], dtype=float)
+    m = np.array([7.0, g["mj"]])  # m_i must not enter
+    acc, jerk, cnt, lists = impl.regular_force(xp, vp, m, np.array([0], dtype=np.int32), np.array([0.0]))
+    np.testing.assert_allclose(acc[0], g["acc"], rtol=0, atol=1e-17)
+    np.testing.assert_allclose(jerk[0], g["jerk"], rtol=0, atol=1e-17)
+    assert cnt[0] == 0 and len(lists[0]) == 0
+    # Newton's third law for the other particle: force on j from i has the opposite direction, weight m_i
+    acc1, jerk1, _, _ = impl.regular_force(xp, vp, m, np.array([1], dtype=np.int32), np.array([0.0]))
+    np.testing.assert_allclose(acc1[0] * m[1], -np.array(g["acc"]) * m[0], rtol=1e-15)
+    np.testing.assert_allclose(jerk1[0] * m[1], -np.array(g["jerk"]) * m[0], rtol=1e-15)
+
+
+# ---------------------------------------------------------------- P2 ring on axis, and the step at r = r_s
+@pytest.mark.parametrize("impl", [oracle, oracle_np])
+def test_p2_ring(impl):
+    g = GOLD["P2_ring"]
+    nr = g["n_ring"]
+    ang = 2 * np.pi * np.arange(nr) / nr
+    xp = np.zeros((nr + 1, 3))
+    xp[:nr, 0] = g["radius"] * np.cos(ang)
+    xp[:nr, 1] = g["radius"] * np.sin(ang)
+    xp[nr] = [0, 0, g["zi"]]
+    vp = np.zeros((nr + 1, 3))
+    vp[nr] = [0, 0, g["wi"]]
+    m = np.full(nr + 1, g["m_each"])
+    ii = np.array([nr], dtype=np.int32)
+    for rs in (0.0, g["rs_inside"]):
+        acc, jerk, cnt, _ = impl.regular_force(xp, vp, m, ii, np.array([rs]))
+        np.testing.assert_allclose(acc[0], g["acc"], atol=1e-16)
+        np.testing.assert_allclose(jerk[0], g["jerk"], atol=1e-16)
+        assert cnt[0] == 0
+    acc, jerk, cnt, lists = impl.regular_force(xp, vp, m, ii, np.array([g["rs_outside"]]))
+    assert cnt[0] == nr and sorted(lists[0]) == list(range(nr))
+    assert np.all(acc == 0.0) and np.all(jerk == 0.0)
+
+
+# ---------------------------------------------------------------- P8 predictor closed form
+@pytest.mark.parametrize("impl", [oracle, oracle_np])
+def test_p8_predictor(impl):
+    g = GOLD["P8_predictor"]
+    x0, v0, a0, j0 = (np.array([g[k]], dtype=float) for k in ("x0", "v0", "a0", "j0"))
+    xp, vp = impl.predict(x0, v0, a0, j0, np.array([g["t0"]]), g["t"])
+    assert np.array_equal(xp[0], g["xp"]) and np.array_equal(vp[0], g["vp"])
+    # dt = 0 is the identity
+    xp, vp = impl.predict(x0, v0, a0, j0, np.array([g["t"]]), g["t"])
+    assert np.array_equal(xp, x0) and np.array_equal(vp, v0)
+
+
+def test_predictor_constant_jerk_motion_and_reversal():
+    """Constant-jerk motion is reproduced exactly by the 3rd-order Taylor step, for any dt sign: predict
+    forward by dt from state at t0, rebuild the exact state at t0+dt, predict back by -dt."""
+    rng = np.random.default_rng(5)
+    n = 200
+    x0, v0, a0, j0 = (rng.normal(size=(n, 3)) for _ in range(4))
+    dt = 2.0 ** -rng.integers(2, 9, n)
+    t = 1.0
+    xp, vp = oracle.predict(x0, v0, a0, j0, t - dt, t)
+    a1 = a0 + j0 * dt[:, None]  # exact acceleration at t for constant jerk
+    # oracle.predict takes one target time t: step back row by row (each row has its own t0 = t - dt)
+    for q in range(0, n, 17):
+        xq, vq = oracle.predict(xp[q:q + 1], vp[q:q + 1], a1[q:q + 1], j0[q:q + 1], np.array([t]), t - dt[q])
+        np.testing.assert_allclose(xq[0], x0[q], rtol=0, atol=1e-14)
+        np.testing.assert_allclose(vq[0], v0[q], rtol=0, atol=1e-14)
+    # each term is present with the right coefficient: derivative structure
+    np.testing.assert_allclose((xp - x0 - v0 * dt[:, None] - a0 * dt[:, None] ** 2 / 2) * 6 / dt[:, None] ** 3, j0,
+                               rtol=1e-6, atol=1e-6)
+    np.testing.assert_allclose((vp - v0 - a0 * dt[:, None]) * 2 / dt[:, None] ** 2, j0, rtol=1e-8, atol=1e-8)
+
+
+# ---------------------------------------------------------------- P3 jerk = d(acc)/dt along the trajectory
+def test_p3_jerk_is_time_derivative_of_force():
+    x, v, m = _plummer(512)
+    idx = np.arange(512, dtype=np.int32)
+    rs = inputs.kth_neighbour_distance(x, idx, 16, brute=True) * 1.0001
+    acc, jerk, cnt, lists = oracle.regular_force(x, v, m, idx, rs)
+    eps = 1e-5
+    ap, _ = oracle.force_given_lists(x + eps * v, v, m, idx, lists)  # mask frozen
+    am, _ = oracle.force_given_lists(x - eps * v, v, m, idx, lists)
+    fd = (ap - am) / (2 * eps)
+    assert _rel(fd, jerk).max() < 1e-6
+
+
+# ---------------------------------------------------------------- P4 antisymmetry
+@pytest.mark.parametrize("rs_uniform", [0.0, 0.15])
+def test_p4_antisymmetry(rs_uniform):
+    x, v, m = _plummer(512)
+    idx = np.arange(512, dtype=np.int32)
+    acc, jerk, cnt, lists = oracle.regular_force(x, v, m, idx, np.full(512, rs_uniform))
+    for f in (acc, jerk):
+        tot = np.linalg.norm((m[:, None] * f).sum(axis=0))
+        assert tot / (m * np.linalg.norm(f, axis=1)).sum() < 1e-14
+    # uniform radius: the neighbour relation is symmetric
+    sets = [set(l.tolist()) for l in lists]
+    for i, s in enumerate(sets):
+        for j in s:
+            assert i in sets[j]
+    if rs_uniform > 0:
+        assert cnt.sum() > 0
+
+
+# ---------------------------------------------------------------- P5 complementarity: regular + listed = total
+def test_p5_complementarity():
+    x, v, m = _plummer(512)
+    idx = np.arange(512, dtype=np.int32)
+    rs = inputs.kth_neighbour_distance(x, idx, 16, brute=True) * 1.0001
+    acc, jerk, cnt, lists = oracle.regular_force(x, v, m, idx, rs)
+    tot_a, tot_j, c0, _ = oracle.regular_force(x, v, m, idx, np.zeros(512))
+    assert c0.sum() == 0 and cnt.min() >= 16
+    for q in range(512):  # irregular part eq. (7)-(8) over the emitted list, written out directly
+        L = lists[q]
+        R = x[L] - x[q]
+        V = v[L] - v[q]
+        r = np.linalg.norm(R, axis=1)
+        rv = (R * V).sum(axis=1)
+        ai = (m[L, None] * R / r[:, None] ** 3).sum(axis=0)
+        ji = (m[L, None] * (V / r[:, None] ** 3 - 3 * rv[:, None] * R / r[:, None] ** 5)).sum(axis=0)
+        assert np.linalg.norm(acc[q] + ai - tot_a[q]) / np.linalg.norm(tot_a[q]) < 1e-12
+        assert np.linalg.norm(jerk[q] + ji - tot_j[q]) / np.linalg.norm(tot_j[q]) < 1e-12
+
+
+# ---------------------------------------------------------------- P6 brute-force lists on tiny N
+def test_p6_bruteforce_lists():
+    rng = np.random.default_rng(11)
+    n = 64
+    x = rng.normal(size=(n, 3))
+    v = rng.normal(size=(n, 3))
+    m = rng.uniform(0.5, 1.5, n)
+    idx = rng.permutation(n).astype(np.int32)[:40]
+    rs = rng.uniform(0.0, 1.5, 40)
+    rs[3] = 0.0
+    _, _, cnt, lists = oracle.regular_force(x, v, m, idx, rs)
+    d2 = ((x[:, None, :] - x[None, :, :]) ** 2).sum(axis=2)
+    for q, i in enumerate(idx):
+        want = [j for j in range(n) if j != i and d2[i, j] < rs[q] * rs[q]]
+        assert lists[q].tolist() == want and cnt[q] == len(want)
+
+
+# ---------------------------------------------------------------- P7 limits, self, coincident particles (R3-R5)
+def test_p7_limits_and_degenerate_cases():
+    x, v, m = _plummer(128)
+    idx = np.arange(128, dtype=np.int32)
+    acc, jerk, cnt, lists = oracle.regular_force(x, v, m, idx, np.full(128, 1e3))
+    assert np.all(cnt == 127) and np.all(acc == 0) and np.all(jerk == 0)
+    for q in range(128):
+        assert q not in lists[q]  # self never listed (R3)
+    # coincident distinct particle: neighbour if r_s > 0, skipped entirely if r_s = 0 (R4)
+    x2 = x.copy()
+    x2[5] = x2[9]
+    acc0, _, cnt0, _ = oracle.regular_force(x2, v, m, np.array([5], dtype=np.int32), np.array([0.0]))
+    assert cnt0[0] == 0 and np.all(np.isfinite(acc0))
+    _, _, cnt1, l1 = oracle.regular_force(x2, v, m, np.array([5], dtype=np.int32), np.array([1e-9]))
+    assert cnt1[0] == 1 and l1[0].tolist() == [9]
+    # duplicates in i_idx give identical rows
+    a, j, c, _ = oracle.regular_force(x, v, m, np.array([7, 7, 3], dtype=np.int32), np.array([0.2, 0.2, 0.2]))
+    assert np.array_equal(a[0], a[1]) and np.array_equal(j[0], j[1]) and c[0] == c[1]
+    # stride smaller than the count: count stays true, wrapper still returns the full set
+    _, _, c2, l2 = oracle.regular_force(x, v, m, idx[:4], np.full(4, 1e3), list_stride=8)
+    assert np.all(c2 == 127) and all(len(l) == 127 for l in l2)
+
+
+# ---------------------------------------------------------------- P9 invariances
+def test_p9_invariances():
+    x, v, m = _plummer(256)
+    idx = np.arange(0, 256, 3, dtype=np.int32)
+    rs = inputs.kth_neighbour_distance(x, idx, 12, brute=True) * 1.0001
+    acc, jerk, cnt, lists = oracle.regular_force(x, v, m, idx, rs)
+    # translation of positions and boost of velocities
+    c, u = np.array([100.0, -50.0, 25.0]), np.array([3.0, -2.0, 1.0])
+    a2, j2, c2, l2 = oracle.regular_force(x + c, v + u, m, idx, rs)
+    assert _rel(a2, acc).max() < 1e-11 and _rel(j2, jerk).max() < 1e-11
+    assert all(np.array_equal(p, q) for p, q in zip(lists, l2))
+    # mass scaling
+    a3, j3, _, _ = oracle.regular_force(x, v, 2.5 * m, idx, rs)
+    assert _rel(a3, 2.5 * acc).max() < 1e-14 and _rel(j3, 2.5 * jerk).max() < 1e-14
+    # length scaling x, v, r_s -> lam: acc -> lam^-2, jerk -> lam^-2
+    lam = 4.0
+    a4, j4, c4, _ = oracle.regular_force(lam * x, lam * v, m, idx, lam * rs)
+    assert _rel(a4, acc / lam ** 2).max() < 1e-14 and _rel(j4, jerk / lam ** 2).max() < 1e-14
+    assert np.array_equal(c4, cnt)
+    # velocity scaling alone: acc unchanged, jerk linear in v
+    a5, j5, _, _ = oracle.regular_force(x, 3.0 * v, m, idx, rs)
+    assert _rel(a5, acc).max() < 1e-15 and _rel(j5, 3.0 * jerk).max() < 1e-14
+    # axis permutation (catches a transposed component)
+    perm = [2, 0, 1]
+    a6, j6, _, _ = oracle.regular_force(x[:, perm], v[:, perm], m, idx, rs)
+    assert _rel(a6, acc[:, perm]).max() < 1e-14 and _rel(j6, jerk[:, perm]).max() < 1e-14
+
+
+# ---------------------------------------------------------------- P10 two independent statements agree
+def test_p10_c_vs_numpy():
+    wl = inputs.make_custom(1500, 300, 20, 64, seed_sub=2, masses="salpeter", brute_rs=True)
+    s = wl.state
+    xp_c, vp_c = oracle.predict(s.x0, s.v0, s.a0, s.j0, s.t0, s.t)
+    xp_n, vp_n = oracle_np.predict(s.x0, s.v0, s.a0, s.j0, s.t0, s.t)
+    np.testing.assert_allclose(xp_c, xp_n, rtol=1e-15, atol=1e-16)
+    np.testing.assert_allclose(vp_c, vp_n, rtol=1e-15, atol=1e-16)
+    a_c, j_c, c_c, l_c = oracle.regular_force(xp_c, vp_c, s.m, wl.i_idx, wl.r_s)
+    a_n, j_n, c_n, l_n = oracle_np.regular_force(xp_c, vp_c, s.m, wl.i_idx, wl.r_s)
+    assert _rel(a_c, a_n).max() < 1e-13 and _rel(j_c, j_n).max() < 1e-13
+    assert np.array_equal(c_c, c_n) and all(np.array_equal(p, q) for p, q in zip(l_c, l_n))
+    # force_given_lists with the oracle's own lists reproduces the regular force bit for bit
+    a_g, j_g = oracle.force_given_lists(xp_c, vp_c, s.m, wl.i_idx, l_c)
+    assert np.array_equal(a_g, a_c) and np.array_equal(j_g, j_c)
+
+
+def test_thread_count_does_not_change_results():
+    x, v, m = _plummer(300)
+    idx = np.arange(300, dtype=np.int32)
+    rs = np.full(300, 0.2)
+    nt = oracle.num_threads()
+    a, j, c, _ = oracle.regular_force(x, v, m, idx, rs)
+    oracle.set_num_threads(1)
+    a1, j1, c1, _ = oracle.regular_force(x, v, m, idx, rs)
+    oracle.set_num_threads(nt)
+    assert np.array_equal(a, a1) and np.array_equal(j, j1) and np.array_equal(c, c1)
