@@ -1,0 +1,123 @@
+/* nbreg.h -- C ABI of the B200-native Ahmad-Cohen regular-force path (after arXiv 1205.1222).
+ *
+ * The library is the GPU counterpart of the paper's GPUNB library: "GPUNB receives positions, velocities,
+ * masses and time-steps of the attracting particles (j-particles) and positions, velocities and neighbour
+ * radii of the attracted (active) particles (i-particles), and it returns regular forces, their time
+ * derivatives and neighbour lists" (section 3.1; calls GPUNB_OPEN / GPUNB_SEND / GPUNB_REGF /
+ * GPUNB_CLOSE at PAPER.md:460,557,595,714).  Differences from GPUNB_REGF: the active block is given as
+ * indices + r_s + t (not pre-packed XI, VI, H2I), and the Hermite predictor of step (iii) (the
+ * host routine CXVPRED at PAPER.md:551-552) runs on the device.
+ *
+ * Conventions
+ *   - Units G = 1.  R_ij = R_j - R_i, V_ij likewise.  acc = + sum m_j R_ij / r^3.
+ *   - "dev" pointers are CUDA device pointers OWNED BY THE CALLER (e.g. PyTorch tensors); "host" pointers are
+ *     ordinary host memory (pinned memory makes the copies asynchronous and fast).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-pointer calls only
+ *     ENQUEUE work on `stream` and return; they never synchronise the host.
+ *   - [n][3] arrays are row-major (x, y, z contiguous per particle).  Indices are 0-based int32.
+ *   - Every function returns NB_OK (0) or a negative NB_E_* code; on error nothing has been enqueued.
+ *     nb_strerror() gives the text; for NB_E_CUDA it includes the CUDA error string of the last failure.
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with NB_E_CUDA.
+ */
+#ifndef NBREG_H_
+#define NBREG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NB_OK 0
+#define NB_E_INVAL (-1) /* null pointer, n > n_max, n_i > n_i_max, negative size, cap <= 0, bad option   */
+#define NB_E_STATE (-2) /* call out of order: force/predict before nb_set_j, get_predicted before predict */
+#define NB_E_NOMEM (-3) /* workspace too small, or a device allocation failed                            */
+#define NB_E_CUDA (-4)  /* CUDA runtime / launch error                                                     */
+
+typedef struct nb_ctx nb_ctx;
+
+/* Library version: major * 10000 + minor * 100 + patch. */
+int nb_version(void);
+
+/* Text for a return code.  The pointer stays valid until the next failing call on the same thread. */
+const char* nb_strerror(int code);
+
+/* Bytes of device workspace nb_create needs for up to n_max j-particles, active blocks of up to n_i_max rows
+ * and neighbour lists of nbr_cap entries per row.  Holds the packed predicted j-records (40 B per j) and, for
+ * the j-split path (small active blocks), per-(row, j-chunk) partial sums, counts and lists.
+ * Returns 0 if an argument is invalid. */
+size_t nb_workspace_bytes(int64_t n_max, int64_t n_i_max, int32_t nbr_cap);
+
+/* cf. GPUNB_OPEN(NTOT).  Creates a context on CUDA device `device`.
+ * dev_workspace: dev pointer to >= nb_workspace_bytes(...) bytes, 256-byte aligned, owned by the caller and
+ * kept alive until nb_destroy; or NULL, in which case the library allocates (and later frees) it itself. */
+int nb_create(nb_ctx** out, int device, int64_t n_max, int64_t n_i_max, int32_t nbr_cap, void* dev_workspace,
+              size_t workspace_bytes);
+
+/* cf. GPUNB_CLOSE.  Frees only what the library allocated itself.  NULL is allowed. */
+int nb_destroy(nb_ctx* ctx);
+
+/* cf. GPUNB_SEND(NN, BODY, X, XDOT), plus CXVPRED's inputs T0, X0, X0DOT, F, FDOT.
+ * Registers the j-particle state WITHOUT copying: the context keeps the six dev pointers until the next
+ * nb_set_j; the arrays must stay alive and unchanged while calls that read them are in flight.
+ *   x0, v0, a0, j0: dev double[n][3]  position, velocity, acceleration, jerk at the particle's own time t0
+ *                                     (physical values, no 1/2 or 1/6 folded in)
+ *   m, t0:          dev double[n]     mass; time of the last force evaluation
+ * Invalidates any earlier prediction.  1 <= n <= n_max. */
+int nb_set_j(nb_ctx* ctx, int64_t n, const double* x0, const double* v0, const double* a0, const double* j0,
+             const double* m, const double* t0);
+
+/* Step (iii): predict all n particles to time t,
+ *   x_p = x0 + v0 dt + a0 dt^2/2 + j0 dt^3/6,  v_p = v0 + a0 dt + j0 dt^2/2,  dt = t - t0[j]  (any sign),
+ * in fp64, and store them as packed records in the workspace: position as a double-single pair of floats
+ * (hi = fl32(x_p), lo = fl32(x_p - hi)), velocity and mass as fl32.  Enqueues one kernel on `stream`. */
+int nb_predict_j(nb_ctx* ctx, double t, void* stream);
+
+/* Test hook: write the fp64 predicted state of the last nb_predict_j / nb_regular_force time to
+ * xp, vp: dev double[n][3].  Same kernel and arithmetic as nb_predict_j. */
+int nb_get_predicted(nb_ctx* ctx, double* xp, double* vp, void* stream);
+
+/* Step (vi), eq. (9), (10), (11), with the plain neighbour criterion eq. (2), PAPER.md:65-67:
+ * for each row q (particle i = i_idx[q], radius r_s[q]) over all j != i,
+ *   neighbour  iff |R_ij|^2 <  r_s^2 : j goes to the list, nothing is summed;
+ *   otherwise                        : acc += m_j R_ij / r^3,  jerk += m_j [V_ij / r^3 - 3 (R_ij.V_ij) R_ij / r^5].
+ * If t differs from the time of the last prediction, nb_predict_j(t) runs first on the same stream (the fused
+ * call).  Differences are formed from the double-single positions, pair arithmetic is fp32 with rsqrt, partial
+ * sums are flushed to fp64 every j-tile; outputs are fp64.
+ *   n_i:        0 <= n_i <= n_i_max (0 is a no-op that only zeroes n_overflow)
+ *   i_idx:      dev int32[n_i]   0-based indices into the j arrays; duplicates allowed
+ *   r_s:        dev double[n_i]  neighbour radius; 0 is legal (empty list, everything summed)
+ *   acc, jerk:  dev double[n_i][3]
+ *   nbr_count:  dev int32[n_i]   TRUE number of neighbours (may exceed nbr_cap: overflow, not an error)
+ *   nbr_list:   dev int32[n_i][nbr_cap]  row q valid in [0, min(count, nbr_cap)), ascending j; the self index
+ *               is never listed or counted; entries past the count are left untouched
+ *   n_overflow: dev int32[1]     number of rows with count > nbr_cap
+ * The pair within 1e-6 (relative) of r_s may fall on either side of the test (fp32 squares). */
+int nb_regular_force(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const double* r_s, double t, double* acc,
+                     double* jerk, int32_t* nbr_count, int32_t* nbr_list, int32_t* n_overflow, void* stream);
+
+/* End-to-end convenience with HOST buffers: copies the j-state and the active block to device buffers the
+ * context owns (allocated on first use, sized by n_max / n_i_max / nbr_cap), runs nb_set_j + nb_regular_force
+ * on an internal stream, copies acc, jerk, nbr_count, nbr_list (n_i x nbr_cap) and n_overflow back and
+ * synchronises.  All pointers are host pointers with the shapes documented above. */
+int nb_regular_force_host(nb_ctx* ctx, int64_t n, const double* x0, const double* v0, const double* a0,
+                          const double* j0, const double* m, const double* t0, int32_t n_i, const int32_t* i_idx,
+                          const double* r_s, double t, double* acc, double* jerk, int32_t* nbr_count,
+                          int32_t* nbr_list, int32_t* n_overflow);
+
+/* Tuning knobs (tests and benchmarks).  key:
+ *   "j_split"   force the number of j-chunks per row (0 = automatic)
+ *   "i_block"   force the rows per CTA: 32, 64, 128, 256 or 512 (0 = automatic)
+ * Returns NB_E_INVAL for an unknown key or value. */
+int nb_set_option(nb_ctx* ctx, const char* key, int64_t value);
+
+/* What the last nb_regular_force enqueued: info[0] rows per CTA, [1] i per thread, [2] j-chunks per row,
+ * [3] grid.x, [4] grid.y, [5] kernels launched by that call (predictor included), [6] j per shared-memory
+ * tile, [7] CTAs per SM the force kernel can hold. */
+int nb_last_launch_info(const nb_ctx* ctx, int64_t info[8]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NBREG_H_ */

@@ -1,0 +1,27 @@
+// nbreg_common.cuh -- shared definitions of the CUDA path (no arithmetic of the method lives here).
+//
+// Packed predicted j-records ("Jparticle" of Listing B1, redesigned): the predictor
+// writes, and the force kernel streams through shared memory, one 80-byte record per PAIR of consecutive
+// j-particles (j0 = 2p, j1 = 2p + 1), laid out so that each 16-byte quarter feeds one packed f32x2
+// instruction operand pair directly:
+//     q0 = { xh0, xh1, yh0, yh1 }     position high words   (xh = fl32(x_p))
+//     q1 = { zh0, zh1, m0,  m1  }
+//     q2 = { xl0, xl1, yl0, yl1 }     position low words    (xl = fl32(x_p - xh): "two-float")
+//     q3 = { zl0, zl1, vx0, vx1 }
+//     q4 = { vy0, vy1, vz0, vz1 }     velocity, fl32
+// = 40 B per j.  The array is padded with massless dummies parked far away up to a multiple of kJPad.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace nbreg {
+
+constexpr int kQuadsPerPair = 5;       // float4 per packed j-pair
+constexpr int kBytesPerJ = 40;         // packed bytes per j-particle
+constexpr int kJPad = 256;             // packed array length is a multiple of this (largest j-tile)
+constexpr float kFarAway = 1.0e18f;    // coordinate of the massless padding particles
+constexpr int64_t kRowChunkLimit = 131072;  // max (rows x j-chunks) the j-split workspace holds
+
+__host__ __device__ inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
+
+}  // namespace nbreg

@@ -1,0 +1,97 @@
+"""GPU-vs-oracle acceptance of BASELINE.json north_star, shared by the -m gpu tests and smoke().
+
+Per active row: |acc_gpu - acc_or| / |acc_or| <= 1e-6, |jerk_gpu - jerk_or| / |jerk_or| <= 1e-5 (Euclidean
+norms).  Neighbour lists equal as SETS, except pairs with |r_ij - r_s| / r_s < 1e-6 (fp64 r), which may fall
+on either side and are reported; rows holding such a pair are force-checked against the oracle re-summed
+with the GPU's list.  Overflowed rows (count > cap): counts equal, stored entries are a
+subset of the true set of size cap (reading R7).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+TOL_ACC = 1e-6
+TOL_JERK = 1e-5
+BAND = 1e-6
+
+
+def relerr(a, b):
+    den = np.linalg.norm(b, axis=-1)
+    den = np.where(den == 0.0, 1.0, den)
+    return np.linalg.norm(a - b, axis=-1) / den
+
+
+def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None):
+    """gpu: dict of numpy arrays acc, jerk, nbr_count, nbr_list, n_overflow (full block).
+    rows: optional subset of row numbers to check (oracle runs only on those).  Returns a report dict;
+    raises AssertionError on a violation."""
+    i_idx = np.asarray(i_idx)
+    if rows is None:
+        rows = np.arange(i_idx.shape[0])
+    rows = np.asarray(rows)
+    sub_idx = np.ascontiguousarray(i_idx[rows], dtype=np.int32)
+    sub_rs = np.ascontiguousarray(r_s[rows])
+    stride = list_stride or max(2 * cap, 64)
+    acc_o, jerk_o, cnt_o, lists_o = oracle.regular_force(xp, vp, m, sub_idx, sub_rs, list_stride=stride)
+    acc_g, jerk_g = gpu["acc"][rows].copy(), gpu["jerk"][rows].copy()
+    cnt_g = gpu["nbr_count"][rows]
+    list_g = gpu["nbr_list"][rows]
+    n_band_pairs, worst_band, n_over = 0, 0.0, 0
+    recheck = []  # rows whose list differs only inside the band
+    for q in range(rows.shape[0]):
+        so = lists_o[q]
+        stored = min(int(cnt_g[q]), cap)
+        sg = list_g[q, :stored]
+        assert np.all(np.diff(sg) > 0), f"row {rows[q]}: GPU list not strictly ascending"
+        if cnt_g[q] > cap or cnt_o[q] > cap:
+            n_over += 1
+        if cnt_g[q] == cnt_o[q] and stored == cnt_o[q] and np.array_equal(sg, so):
+            continue
+        set_o, set_g = set(so.tolist()), set(sg.tolist())
+        if cnt_g[q] > cap:  # overflowed row: only `cap` entries are stored
+            diff = set_g - set_o
+            extra_needed = int(cnt_g[q]) != int(cnt_o[q])
+        else:
+            diff = set_g ^ set_o
+            extra_needed = True
+        if not diff and not extra_needed:
+            continue
+        # every disagreeing j must sit inside the boundary band
+        i = sub_idx[q]
+        if cnt_g[q] > cap and not diff:
+            # counts differ on an overflowed row: cannot name the pair; bound the number of band pairs instead
+            d = np.linalg.norm(xp - xp[i], axis=1)
+            nband = int((np.abs(d - sub_rs[q]) < BAND * sub_rs[q]).sum())
+            assert abs(int(cnt_g[q]) - int(cnt_o[q])) <= nband, f"row {rows[q]}: overflow count mismatch"
+            n_band_pairs += abs(int(cnt_g[q]) - int(cnt_o[q]))
+            continue
+        for j in diff:
+            d = np.linalg.norm(xp[j] - xp[i])
+            off = abs(d - sub_rs[q]) / sub_rs[q]
+            assert off < BAND, f"row {rows[q]} (i={i}): list differs at j={j}, |r-r_s|/r_s={off:.3e} outside band"
+            worst_band = max(worst_band, off)
+            n_band_pairs += 1
+        if cnt_g[q] <= cap:
+            assert int(cnt_g[q]) == len(set_g)
+            recheck.append(q)
+    if recheck:  # H4: force parity against the oracle re-summed with the GPU's own list
+        rq = np.array(recheck)
+        a2, j2 = oracle.force_given_lists(xp, vp, m, sub_idx[rq], [list_g[q, : cnt_g[q]] for q in rq])
+        acc_o[rq], jerk_o[rq] = a2, j2
+    ea, ej = relerr(acc_g, acc_o), relerr(jerk_g, jerk_o)
+    # rows where everything is a neighbour have acc = jerk = 0 exactly on both sides
+    zero = (np.linalg.norm(acc_o, axis=1) == 0)
+    if zero.any():
+        assert np.all(acc_g[zero] == 0) and np.all(jerk_g[zero] == 0)
+    worst_a = int(np.argmax(ea))
+    assert ea.max() <= TOL_ACC, f"acc rel err {ea.max():.3e} at row {rows[worst_a]} > {TOL_ACC}"
+    assert ej.max() <= TOL_JERK, f"jerk rel err {ej.max():.3e} at row {rows[int(np.argmax(ej))]} > {TOL_JERK}"
+    return dict(rows=int(rows.shape[0]), max_acc_err=float(ea.max()), max_jerk_err=float(ej.max()),
+                median_acc_err=float(np.median(ea)), band_pairs=int(n_band_pairs), worst_band=float(worst_band),
+                overflow_rows=int(n_over), mean_count=float(cnt_o.mean()))
+
+
+def check_overflow_flag(gpu, cap):
+    n_over = int((gpu["nbr_count"] > cap).sum())
+    assert int(gpu["n_overflow"][0]) == n_over, (int(gpu["n_overflow"][0]), n_over)
+    return n_over

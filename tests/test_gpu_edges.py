@@ -1,0 +1,148 @@
+"""Edge cases of the CUDA path against the oracle (-m gpu): ragged sizes, every CTA shape and j-split,
+degenerate radii, overflow, duplicates, translation, coincident particles, host-buffer entry point."""
+import ctypes
+
+import numpy as np
+import pytest
+import torch
+
+from paper_1205_1222_b200 import binding, inputs
+import parity
+from gpu_util import run_gpu
+
+pytestmark = pytest.mark.gpu
+
+
+def _wl(oracle, n, n_i, k, cap, **kw):
+    return inputs.make_custom(n, n_i, k, cap, predict=lambda s: oracle.predict_state(s)[0], **kw)
+
+
+def _full_check(oracle, wl, gpu, cap=None):
+    xp, vp = oracle.predict_state(wl.state)
+    rep = parity.compare(oracle, xp, vp, wl.state.m, wl.i_idx, wl.r_s, cap or wl.cap, gpu)
+    parity.check_overflow_flag(gpu, cap or wl.cap)
+    return rep
+
+
+@pytest.mark.parametrize("i_block", [32, 64, 128, 256, 512])
+@pytest.mark.parametrize("j_split", [1, 3, 0])
+def test_every_cta_shape_and_split_ragged(oracle, i_block, j_split):
+    # n odd and not a multiple of any tile; n_i not a multiple of any CTA width; several tiles per chunk
+    wl = _wl(oracle, 2999, 777, 24, 64, masses="salpeter")
+    gpu, info = run_gpu(wl, options={"i_block": i_block, "j_split": j_split})
+    assert info["rows_per_cta"] == i_block and (j_split == 0 or info["j_chunks"] == j_split)
+    _full_check(oracle, wl, gpu)
+
+
+def test_shapes_and_splits_agree_bitwise_on_lists_and_closely_on_sums(oracle):
+    wl = _wl(oracle, 4096, 512, 30, 64)
+    ref, _ = run_gpu(wl, options={"i_block": 256, "j_split": 1})
+    for ib, sp in ((32, 7), (128, 2), (512, 1)):
+        g, _ = run_gpu(wl, options={"i_block": ib, "j_split": sp})
+        assert np.array_equal(g["nbr_count"], ref["nbr_count"])
+        for q in range(wl.n_i):
+            c = ref["nbr_count"][q]
+            assert np.array_equal(g["nbr_list"][q, :c], ref["nbr_list"][q, :c])
+        assert parity.relerr(g["acc"], ref["acc"]).max() < 5e-7
+
+
+def test_deterministic_repeat(oracle):
+    wl = _wl(oracle, 5000, 300, 20, 64)
+    a, _ = run_gpu(wl)
+    b, _ = run_gpu(wl)
+    for k in ("acc", "jerk", "nbr_count", "n_overflow"):
+        assert np.array_equal(a[k], b[k])
+
+
+def test_degenerate_radii_and_tiny_blocks(oracle):
+    wl = _wl(oracle, 1500, 64, 16, 32)
+    # r_s = 0: empty list, total force; r_s huge: everything a neighbour, zero force, overflow
+    wl.r_s[:8] = 0.0
+    wl.r_s[8:12] = 1e3
+    gpu, _ = run_gpu(wl)
+    rep = _full_check(oracle, wl, gpu)
+    assert np.all(gpu["nbr_count"][:8] == 0)
+    assert np.all(gpu["nbr_count"][8:12] == wl.state.n - 1)
+    assert np.all(gpu["acc"][8:12] == 0) and np.all(gpu["jerk"][8:12] == 0)
+    assert int(gpu["n_overflow"][0]) >= 4 and rep["overflow_rows"] >= 4
+    # n_i = 1 and n_i = 0
+    one = inputs.Workload(wl.state, wl.i_idx[20:21].copy(), wl.r_s[20:21].copy(), wl.k, wl.cap)
+    g1, _ = run_gpu(one)
+    assert np.array_equal(g1["acc"][0], gpu["acc"][20]) or parity.relerr(g1["acc"], gpu["acc"][20:21]).max() < 5e-7
+    _full_check(oracle, one, g1)
+    zero = inputs.Workload(wl.state, wl.i_idx[:0].copy(), wl.r_s[:0].copy(), wl.k, wl.cap)
+    g0, _ = run_gpu(zero)
+    assert int(g0["n_overflow"][0]) == 0
+
+
+def test_duplicate_indices_and_self_exclusion(oracle):
+    wl = _wl(oracle, 1200, 96, 12, 32)
+    wl.i_idx[1] = wl.i_idx[0]
+    wl.r_s[1] = wl.r_s[0]
+    gpu, _ = run_gpu(wl)
+    _full_check(oracle, wl, gpu)
+    assert np.array_equal(gpu["acc"][0], gpu["acc"][1]) and gpu["nbr_count"][0] == gpu["nbr_count"][1]
+    for q in range(wl.n_i):
+        assert wl.i_idx[q] not in gpu["nbr_list"][q, : min(gpu["nbr_count"][q], wl.cap)]
+
+
+def test_translation_by_100_needs_double_single(oracle):
+    """with plain fp32 positions this fails by orders of magnitude."""
+    wl = _wl(oracle, 4000, 500, 40, 128)
+    g0, _ = run_gpu(wl)
+    wl.state.x0 = wl.state.x0 + np.array([100.0, -100.0, 50.0])
+    g1, _ = run_gpu(wl)
+    _full_check(oracle, wl, g1)
+    assert parity.relerr(g1["acc"], g0["acc"]).max() < 1e-6
+    same = sum(np.array_equal(g0["nbr_list"][q, :g0["nbr_count"][q]], g1["nbr_list"][q, :g1["nbr_count"][q]])
+               for q in range(wl.n_i))
+    assert same >= wl.n_i - 2
+
+
+def test_coincident_particles(oracle):
+    wl = _wl(oracle, 800, 800, 10, 32, active="all")
+    s = wl.state
+    s.x0[5] = s.x0[9]
+    s.v0[5], s.a0[5], s.j0[5], s.t0[5] = s.v0[9], s.a0[9], s.j0[9], s.t0[9]  # stay coincident after prediction
+    wl.r_s[5] = 0.0      # R4: singular term skipped, not listed
+    wl.r_s[9] = 1e-3     # neighbour (0 < r_s^2)
+    gpu, _ = run_gpu(wl)
+    assert gpu["nbr_count"][5] == 0 and np.all(np.isfinite(gpu["acc"][5]))
+    assert 5 in gpu["nbr_list"][9, : gpu["nbr_count"][9]]
+    _full_check(oracle, wl, gpu)
+
+
+def test_host_entry_point_matches_device_entry_point(oracle):
+    wl = _wl(oracle, 3001, 257, 20, 64)
+    dev_out, _ = run_gpu(wl)
+    s = wl.state
+    ctx = binding.Context(s.n, wl.n_i, wl.cap)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    out = dict(acc=torch.empty((wl.n_i, 3), dtype=torch.float64).pin_memory(),
+               jerk=torch.empty((wl.n_i, 3), dtype=torch.float64).pin_memory(),
+               nbr_count=torch.empty(wl.n_i, dtype=torch.int32).pin_memory(),
+               nbr_list=torch.empty((wl.n_i, wl.cap), dtype=torch.int32).pin_memory(),
+               n_overflow=torch.zeros(1, dtype=torch.int32).pin_memory())
+    ctx.nb_regular_force_host(pin(s.x0), pin(s.v0), pin(s.a0), pin(s.j0), pin(s.m), pin(s.t0),
+                              pin(wl.i_idx.astype(np.int32)), pin(wl.r_s), s.t, out)
+    for k in ("acc", "jerk", "nbr_count"):
+        assert np.array_equal(out[k].numpy(), dev_out[k]), k
+    for q in range(wl.n_i):
+        c = dev_out["nbr_count"][q]
+        assert np.array_equal(out["nbr_list"].numpy()[q, :c], dev_out["nbr_list"][q, :c])
+    ctx.close()
+
+
+def test_error_codes_on_device():
+    lib = binding.load()
+    ctx = binding.Context(1000, 100, 16)
+    dummy = torch.zeros(8, dtype=torch.int32, device="cuda")
+    p = ctypes.c_void_p(dummy.data_ptr())
+    # force before set_j -> NB_E_STATE; n_i > n_i_max -> NB_E_INVAL; null n_overflow -> NB_E_INVAL
+    assert lib.nb_regular_force(ctx._h, 4, p, p, 1.0, p, p, p, p, p, None) == -2
+    assert lib.nb_regular_force(ctx._h, 101, p, p, 1.0, p, p, p, p, p, None) == -1
+    assert lib.nb_regular_force(ctx._h, 4, p, p, 1.0, p, p, p, p, None, None) == -1
+    assert lib.nb_predict_j(ctx._h, 1.0, None) == -2
+    with pytest.raises(binding.NbregError):
+        ctx.nb_set_option("no_such_option", 1)
+    ctx.close()
