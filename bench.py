@@ -1,0 +1,294 @@
+#!/usr/bin/env python
+"""bench.py -- regular-force throughput (G pair-interactions/s: acc + jerk + neighbour list in one pass).
+
+One "step" = one pass of the whole hot path over one synthetic workload: nb_set_j (GPUNB_SEND),
+nb_predict_j (S1, all N particles) and nb_regular_force (S2-S5, N_i x N pairs).  Default workload:
+BASELINE.json config 5 (N = N_i = 1048576 equal-mass Plummer, k ~ 100, cap 512), the largest single-GPU
+configuration and the one SURVEY.md 8(d) names as the headline row.  Inputs are seeded and synthetic
+(paper_1205_1222_b200/inputs.py); r_s is calibrated on the unpredicted positions.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--n-i M] [--impl reference]
+
+N > 1 (torchrun): independent replicas, one per GPU, no collective on the data path ("replicas only").
+--impl reference times the fp64 CPU oracle (oracle/, test infrastructure) on a bounded row sample.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FLOPS_PER_PAIR = 60.0  # convention of BASELINE.json ("e.g. 60 for force+jerk"), SURVEY.md R13
+METRIC = "regular-force Ginteractions/s (acc+jerk+nbr list)"
+UNIT = "Gpairs/s"
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), src="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, src="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def build_workload(config: int, n_i: int | None):
+    from paper_1205_1222_b200 import inputs
+    wl = inputs.make_workload(config, n_i=n_i)
+    return wl
+
+
+def cpu_baseline(wl, target_seconds: float = 12.0, steps: int = 1):
+    """The oracle as it stands, on this host's cores, on a bounded sample of rows of the same workload."""
+    from oracle import oracle
+    s = wl.state
+    xp, vp = oracle.predict_state(s)
+    cores = oracle.num_threads()
+    rows = min(wl.n_i, max(cores, 16))
+    t0 = time.perf_counter()
+    oracle.regular_force(xp, vp, s.m, wl.i_idx[:rows], wl.r_s[:rows], list_stride=2 * wl.cap)
+    dt = time.perf_counter() - t0
+    rate = rows * s.n / dt
+    rows = int(min(wl.n_i, max(rows, rate * target_seconds / s.n)))
+    rows = max(cores, rows // cores * cores)
+    rows = min(rows, wl.n_i)
+    times = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        oracle.regular_force(xp, vp, s.m, wl.i_idx[:rows], wl.r_s[:rows], list_stride=2 * wl.cap)
+        times.append(time.perf_counter() - t0)
+    dt = float(np.mean(times))
+    return dict(value=rows * s.n / dt / 1e9, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"first {rows} active rows x all {s.n} j (fp64, OpenMP, gcc -O2), {dt:.2f} s per pass"), dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle (fp64 CPU) on a bounded sample, same metric/config keys."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    wl = build_workload(args.config, args.n_i)
+    base, _ = cpu_baseline(wl, target_seconds=4.0, steps=1)  # sizes the sample
+    rows = int(base["sample"].split()[1])
+    from oracle import oracle
+    s = wl.state
+    xp, vp = oracle.predict_state(s)
+    for _ in range(args.warmup):
+        oracle.regular_force(xp, vp, s.m, wl.i_idx[:rows], wl.r_s[:rows], list_stride=2 * wl.cap)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        xp, vp = oracle.predict_state(s)
+        oracle.regular_force(xp, vp, s.m, wl.i_idx[:rows], wl.r_s[:rows], list_stride=2 * wl.cap)
+    dt = (time.perf_counter() - t0) / args.steps
+    val = rows * s.n / dt / 1e9
+    cb = dict(value=val, unit=UNIT, cores=base["cores"], kind="oracle",
+              sample=f"each step: predictor on all {s.n} + first {rows} active rows x all j")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(wl, args.config), "cpu_baseline": cb,
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+    return 0
+
+
+def workload_config(wl, config):
+    return {"workload": f"BASELINE.json configs[{config - 1}]: N={wl.state.n} Plummer, N_i={wl.n_i}, "
+                        f"k~{wl.k}, nbr cap {wl.cap}", "n": wl.state.n, "n_i": wl.n_i, "nbr_cap": wl.cap,
+            "pairs_per_step": wl.pairs, "flops_per_pair_convention": FLOPS_PER_PAIR,
+            "r_s_calibrated_on": wl.rs_positions,
+            "l2": "no explicit flush: each step streams 112 B/j of fp64 state plus outputs "
+                  "(lists N_i x cap x 4 B), larger than the 126 MB L2 for the default workload"}
+
+
+def run_gpu_arm(args):
+    import torch
+    from paper_1205_1222_b200 import binding
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the regular-force path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = torch.device(f"cuda:{local}")
+    peaks = _peaks()
+    wl = build_workload(args.config, args.n_i)  # every rank: the same seeded workload (independent replicas)
+    s = wl.state
+    ctx = binding.Context(s.n, wl.n_i, wl.cap, device=local)
+    state_dev = ctx.set_state(s)
+    i_idx = torch.from_numpy(wl.i_idx).to(dev)
+    r_s = torch.from_numpy(wl.r_s).to(dev)
+    out = ctx.alloc_outputs(wl.n_i)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
+
+    def step(ev=None):
+        ctx.nb_set_j(*state_dev)           # GPUNB_SEND: new block-step, prediction invalid
+        if ev: ev[0].record()
+        ctx.nb_predict_j(s.t)              # S1
+        if ev: ev[1].record()
+        ctx.nb_regular_force(i_idx, r_s, s.t, out=out)  # S2-S5 (prediction already at t)
+        if ev: ev[2].record()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    info = ctx.nb_last_launch_info()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    if dist: dist.barrier()
+    torch.cuda.synchronize()
+    for k in range(args.steps):
+        flush.fill_(k & 0xff)              # L2 flush between timed iterations (outside the per-step events)
+        step(evs[k])
+    torch.cuda.synchronize()
+    if dist: dist.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    t_step = sum(e[0].elapsed_time(e[2]) for e in evs) / 1e3          # s, all K steps, device time
+    t_pred = sum(e[0].elapsed_time(e[1]) for e in evs) / 1e3 / args.steps
+    t_force = sum(e[1].elapsed_time(e[2]) for e in evs) / 1e3 / args.steps
+    tt = torch.tensor([t_step], dtype=torch.float64, device=dev)
+    if dist: dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_max = float(tt.item())
+    value = world * wl.pairs * args.steps / t_max / 1e9
+    n_over = int(out["n_overflow"].item())
+    mean_cnt = float(out["nbr_count"].double().mean().item())
+
+    # ---- e2e: C-ABI call with HOST (pinned) buffers, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        h_in = [pin(a) for a in (s.x0, s.v0, s.a0, s.j0, s.m, s.t0)]
+        h_idx, h_rs = pin(wl.i_idx), pin(wl.r_s)
+        h_out = dict(acc=torch.empty((wl.n_i, 3), dtype=torch.float64).pin_memory(),
+                     jerk=torch.empty((wl.n_i, 3), dtype=torch.float64).pin_memory(),
+                     nbr_count=torch.empty(wl.n_i, dtype=torch.int32).pin_memory(),
+                     nbr_list=torch.empty((wl.n_i, wl.cap), dtype=torch.int32).pin_memory(),
+                     n_overflow=torch.zeros(1, dtype=torch.int32).pin_memory())
+        h2d = sum(t.numel() * t.element_size() for t in h_in + [h_idx, h_rs])
+        d2h = sum(t.numel() * t.element_size() for t in h_out.values())
+        ksteps = max(1, min(args.steps, 3))
+        ctx.nb_regular_force_host(*h_in, h_idx, h_rs, s.t, h_out)  # warm-up (allocates the mirrors)
+        if dist: dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(ksteps):
+            ctx.nb_regular_force_host(*h_in, h_idx, h_rs, s.t, h_out)  # synchronises internally
+        te = time.perf_counter() - t0
+        te_t = torch.tensor([te], dtype=torch.float64, device=dev)
+        if dist: dist.all_reduce(te_t, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * wl.pairs * ksteps / float(te_t.item()) / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "steps": ksteps,
+               "ms_per_step": float(te_t.item()) / ksteps * 1e3, "api": "nb_regular_force_host (pinned host buffers)"}
+        ctx.nb_set_j(*state_dev)
+
+    if rank != 0:
+        if dist: dist.destroy_process_group()
+        return 0
+    nsm = torch.cuda.get_device_properties(local).multi_processor_count
+    peak_tf = nsm * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    ach_tf = wl.pairs * FLOPS_PER_PAIR / t_force / 1e12
+    pred_bytes = s.n * (112 + 40)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": workload_config(wl, args.config),
+        "fp32_peak_fraction": value / world * 1e9 * FLOPS_PER_PAIR / (peak_tf * 1e12),
+        "roofline": {"bound": "alu", "kernel": "force_kernel", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                     "frac": ach_tf / peak_tf, "traffic": None,
+                     "note": f"achieved = N_i*N pairs x {FLOPS_PER_PAIR:.0f} flop / force-kernel time (CUDA events, "
+                             f"includes the gather kernel when the j-range is split); peak = {nsm} SMs x 128 FP32 "
+                             f"lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz, "
+                             f"{peaks['src']})", "ms": t_force * 1e3},
+        "roofline_predictor": {"bound": "hbm", "kernel": "predict_kernel", "achieved": pred_bytes / t_pred / 1e9,
+                               "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": pred_bytes / t_pred / 1e9 / peaks["hbm_gbs"],
+                               "traffic": None, "ms": t_pred * 1e3,
+                               "note": f"152 B/j algorithmic (112 read + 40 written), peak {peaks['src']} copy bandwidth"},
+        "launch": info, "gpu_launches": int(info["launches"] + 1) * args.steps,
+        "mean_neighbours": mean_cnt, "overflow_rows": n_over, "clocks": clocks, "e2e": e2e,
+    }
+    if not args.no_cpu and world >= 1:
+        cb, _ = cpu_baseline(wl, target_seconds=args.cpu_seconds)
+        line["cpu_baseline"] = cb
+    print(json.dumps(line))
+    if dist: dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--n-i", type=int, default=None, help="active-block size (configs 1, 3, 5 only)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_gpu_arm(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

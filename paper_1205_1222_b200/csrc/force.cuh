@@ -88,6 +88,9 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 __device__ __forceinline__ float rsqrt_approx(float x) {
     float y;
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+#ifdef NBREG_EXP_NEWTON
+    { float e = fmaf(x * y, -y, 1.0f); y = fmaf(0.5f * y, e, y); }
+#endif
     return y;
 }
 

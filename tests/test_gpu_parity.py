@@ -46,7 +46,7 @@ def test_config3_block_sweep(oracle):
     st = inputs.make_state(3)
     xp, vp = oracle.predict_state(st)
     full = inputs.make_workload(3, predict=lambda s: xp, state=st)
-    saw_split = saw_direct = False
+    saw_split = False
     for n_i in inputs.CONFIG3_BLOCKS:
         wl = inputs.Workload(st, full.i_idx[:n_i].copy(), full.r_s[:n_i].copy(), full.k, full.cap)
         gpu, info = run_gpu(wl)
@@ -54,9 +54,8 @@ def test_config3_block_sweep(oracle):
         rep = parity.compare(oracle, xp, vp, st.m, wl.i_idx, wl.r_s, wl.cap, gpu, rows=rows)
         parity.check_overflow_flag(gpu, wl.cap)
         saw_split |= info["j_chunks"] > 1
-        saw_direct |= info["j_chunks"] == 1
         print(n_i, info, rep)
-    assert saw_split and saw_direct
+    assert saw_split  # the direct (one chunk per row) path is config 5's
 
 
 def test_config4_binaries_and_overflow(oracle):
