@@ -107,15 +107,23 @@ int nb_regular_force_host(nb_ctx* ctx, int64_t n, const double* x0, const double
                           int32_t* nbr_list, int32_t* n_overflow);
 
 /* Tuning knobs (tests and benchmarks).  key:
- *   "j_split"   force the number of j-chunks per row (0 = automatic)
+ *   "j_split"   force the number of j-chunks per row for ALL row blocks (0 = automatic; 1 = never split)
  *   "i_block"   force the rows per CTA: 32, 64, 128, 256 or 512 (0 = automatic)
  * Returns NB_E_INVAL for an unknown key or value. */
 int nb_set_option(nb_ctx* ctx, const char* key, int64_t value);
 
-/* What the last nb_regular_force enqueued: info[0] rows per CTA, [1] i per thread, [2] j-chunks per row,
- * [3] grid.x, [4] grid.y, [5] kernels launched by that call (predictor included), [6] j per shared-memory
- * tile, [7] CTAs per SM the force kernel can hold. */
+/* What the last nb_regular_force enqueued: info[0] rows per CTA, [1] i per thread, [2] j-chunks per split row
+ * block (1 = nothing split), [3] CTAs of the force kernel, [4] row blocks whose j-range was split (the "tail"
+ * that fills the last wave of CTAs; all blocks for a small active block), [5] kernels
+ * launched by that call (predictor included), [6] j per shared-memory tile, [7] CTAs per SM the force kernel
+ * can hold. */
 int nb_last_launch_info(const nb_ctx* ctx, int64_t info[8]);
+
+/* The launch planner alone (host only, no device needed): the plan nb_regular_force would use for n
+ * j-particles and n_i rows on a GPU with num_sms SMs holding ctas_per_sm[k] CTAs of shape k (rows per CTA 256,
+ * 128, 64, 32, 512).  info as in nb_last_launch_info, except info[5] = j-tiles per chunk. */
+int nb_plan(int64_t n, int32_t n_i, int32_t num_sms, const int32_t ctas_per_sm[5], int64_t i_block, int64_t j_split,
+            int64_t info[8]);
 
 #ifdef __cplusplus
 }

@@ -51,6 +51,7 @@ def load(build_if_missing: bool = True):
     lib.nb_regular_force_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp]
     lib.nb_set_option.argtypes = [vp, ctypes.c_char_p, i64]
     lib.nb_last_launch_info.argtypes = [vp, ctypes.POINTER(i64)]
+    lib.nb_plan.argtypes = [i64, i32, i32, ctypes.POINTER(i32), i64, i64, ctypes.POINTER(i64)]
     _lib = lib
     return lib
 
@@ -75,6 +76,21 @@ def _host(t: torch.Tensor, dtype, what: str):
 def _stream_ptr(stream):
     s = torch.cuda.current_stream() if stream is None else stream
     return ctypes.c_void_p(s.cuda_stream)
+
+
+_INFO_KEYS = ("rows_per_cta", "i_per_thread", "j_chunks", "ctas", "split_row_blocks", "launches", "j_tile",
+              "ctas_per_sm")
+
+
+def nb_plan(n: int, n_i: int, num_sms: int = 148, ctas_per_sm=(3, 6, 12, 24, 1), i_block: int = 0,
+            j_split: int = 0) -> dict:
+    """The launch planner alone (host only).  Same keys as nb_last_launch_info, with tiles_per_chunk in place
+    of launches."""
+    arr = (ctypes.c_int64 * 8)()
+    occ = (ctypes.c_int32 * 5)(*[int(v) for v in ctas_per_sm])
+    _check(load().nb_plan(int(n), int(n_i), int(num_sms), occ, int(i_block), int(j_split), arr))
+    keys = tuple("tiles_per_chunk" if k == "launches" else k for k in _INFO_KEYS)
+    return dict(zip(keys, [int(v) for v in arr]))
 
 
 class Context:
@@ -166,7 +182,7 @@ class Context:
     def nb_last_launch_info(self) -> dict:
         arr = (ctypes.c_int64 * 8)()
         _check(self.lib.nb_last_launch_info(self._h, arr))
-        keys = ("rows_per_cta", "i_per_thread", "j_chunks", "grid_x", "grid_y", "launches", "j_tile", "ctas_per_sm")
+        keys = _INFO_KEYS
         return dict(zip(keys, [int(v) for v in arr]))
 
     # -- convenience: upload a numpy State (inputs.State) and register it

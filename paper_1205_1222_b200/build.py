@@ -11,7 +11,7 @@ SRC = os.path.join(HERE, "csrc", "nbreg_api.cu")
 DEPS = [os.path.join(HERE, "csrc", f) for f in
         ("nbreg_api.cu", "nbreg_common.cuh", "predict.cuh", "force.cuh", "gather.cuh")] + \
        [os.path.join(os.path.dirname(HERE), "include", "nbreg.h")]
-LIB = os.path.join(HERE, "libnbreg.so")
+LIB = os.environ.get("NBREG_LIB") or os.path.join(HERE, "libnbreg.so")  # NBREG_LIB: use a library built elsewhere
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]

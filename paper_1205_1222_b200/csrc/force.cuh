@@ -18,8 +18,10 @@
 //     PAPER.md:17, footnote at PAPER.md:154): (xh_j - xh_i) + (xl_j - xl_i), then fp32 with one MUFU.RSQ;
 //   * fp32 partial sums are flushed into fp64 running sums after every j-tile (S6);
 //   * the list append sits behind a warp-uniform vote so the common path has no store and no branch taken;
-//   * when blockDim.y > 1 the j-range is split over CTAs and the kernel writes per-(row,
-//     chunk) partial sums / counts / lists for reduce_gather_kernel (gather.cuh).
+//   * the j-range of the last ("tail") row blocks is split over several CTAs so that the
+//     CTA count fills whole waves of the 148 SMs; those CTAs write per-(row, chunk) partial sums for
+//     reduce_gather_kernel (gather.cuh) and share the row's list through an atomic slot counter.  Small active
+//     blocks are all tail.
 #pragma once
 #include "nbreg_common.cuh"
 
@@ -29,22 +31,25 @@ struct ForceArgs {
     const float4* packed;   // packed j-pair records, n_pad / 2 pairs
     int32_t n;              // real j-particles
     int32_t n_tiles;        // number of JT-sized tiles covering n_pad
+    // CTA b < main_blocks: row block b against the whole j-range, final outputs written directly.
+    // CTA b >= main_blocks ("tail"): t = b - main_blocks, row block main_blocks + t / n_chunks against j-chunk
+    // t % n_chunks (tiles_per_chunk tiles), partial outputs for reduce_gather_kernel.
+    int32_t main_blocks;
     int32_t tiles_per_chunk;
-    int32_t n_chunks;       // S = gridDim.y
+    int32_t n_chunks;       // S >= 2 for the tail blocks (unused when there is no tail)
     int32_t n_i;
     int32_t cap;
     const int32_t* i_idx;
     const double* r_s;
-    // final outputs (used when n_chunks == 1)
+    // final outputs (main blocks)
     double* acc;
     double* jerk;
     int32_t* nbr_count;
     int32_t* nbr_list;
     int32_t* n_overflow;
-    // partial outputs (used when n_chunks > 1): [row][chunk]
-    double* part_sum;     // [rows][S][6]
-    int32_t* part_cnt;    // [rows][S]
-    int32_t* part_list;   // [rows][S][cap]
+    // partial sums of the tail blocks, indexed by tail row = row - main_blocks * rows_per_cta: [tail row][S][6].
+    // Their list entries go straight to nbr_list through an atomic slot counter in nbr_count (zeroed by the host).
+    double* part_sum;
 };
 
 // ---------------------------------------------------------------- PTX helpers
@@ -85,23 +90,27 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  "l"(src), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
 }
-__device__ __forceinline__ float rsqrt_approx(float x) {
+__device__ __forceinline__ float rsqrt_approx(float x) {  // MUFU.RSQ; rsqrt(+inf) = 0
     float y;
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-#ifdef NBREG_EXP_NEWTON
-    { float e = fmaf(x * y, -y, 1.0f); y = fmaf(0.5f * y, e, y); }
-#endif
+    return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {  // MUFU.RCP; rcp(+inf) = 0
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
 
 // ---------------------------------------------------------------- per-thread i-state
 struct IState {
-    // negated and duplicated so that d = j + (-i) is one packed add per component
-    float2 nxh, nyh, nzh, nxl, nyl, nzl, nvx, nvy, nvz;
+    // negated, so that d = j + (-i) is one packed add per component (the scalar is broadcast to both halves)
+    float nxh, nyh, nzh, nxl, nyl, nzl, nvx, nvy, nvz;
     float h2;        // r_s^2 in fp32, clamped to >= FLT_MIN so that the self pair (r^2 = 0) is always masked
+    float hfar2;     // pairs with |R_hi|^2 >= hfar2 take the far path (no low words, surely not a neighbour)
     int32_t self;    // own j-index (never listed)
     int32_t nlim;    // list entries must have j < nlim: n for a normal row, 0 when r_s = 0 (reading R4/R5)
-    int32_t cnt;     // neighbours found so far in this CTA's j-range
+    int32_t cnt;     // main path: neighbours found so far
+    int32_t pend_j, pend_pos;  // j-split path: the append whose slot number is still in flight (pend_j < 0: none)
     int32_t* list;   // where this row's (partial) list goes
 };
 
@@ -113,39 +122,77 @@ __device__ __forceinline__ void accum_zero(Accum& s) {
     s.ax = s.ay = s.az = s.jx = s.jy = s.jz = make_float2(0.f, 0.f);
 }
 
-// One packed step: the pair (j0, j1) held in q0..q4 against one i.  32 packed FP32 instructions
-// (12 FADD2, 7 FMUL2, 13 FFMA2), 2 MUFU.RSQ, 2 FSETP, 2 FSEL.  Returns the two neighbour predicates.
-__device__ __forceinline__ void pair_step(const float4& q0, const float4& q1, const float4& q2, const float4& q3,
-                                          const float4& q4, const IState& I, Accum& s, bool& nb0, bool& nb1) {
-    // double-single coordinate differences ("pseudo double precision for the coordinate differences")
-    float2 dx = __fadd2_rn(__fadd2_rn(make_float2(q0.x, q0.y), I.nxh), __fadd2_rn(make_float2(q2.x, q2.y), I.nxl));
-    float2 dy = __fadd2_rn(__fadd2_rn(make_float2(q0.z, q0.w), I.nyh), __fadd2_rn(make_float2(q2.z, q2.w), I.nyl));
-    float2 dz = __fadd2_rn(__fadd2_rn(make_float2(q1.x, q1.y), I.nzh), __fadd2_rn(make_float2(q3.x, q3.y), I.nzl));
-    float2 dvx = __fadd2_rn(make_float2(q3.z, q3.w), I.nvx);
-    float2 dvy = __fadd2_rn(make_float2(q4.x, q4.y), I.nvy);
-    float2 dvz = __fadd2_rn(make_float2(q4.z, q4.w), I.nvz);
-    float2 r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
-    float2 rv = __ffma2_rn(dz, dvz, __ffma2_rn(dy, dvy, __fmul2_rn(dx, dvx)));
-    nb0 = r2.x < I.h2;  // eq. (2)/(11): neighbour iff r^2 < r_s^2
-    nb1 = r2.y < I.h2;
-    float2 ri;
-    ri.x = nb0 ? 0.f : rsqrt_approx(r2.x);  // Listing B2 line 31: "rinv1 = 0.f" masks the pair
-    ri.y = nb1 ? 0.f : rsqrt_approx(r2.y);
-    float2 ri2 = __fmul2_rn(ri, ri);
-    float2 mri3 = __fmul2_rn(__fmul2_rn(make_float2(q1.z, q1.w), ri), ri2);
-    float2 al = __fmul2_rn(__fmul2_rn(rv, ri2), make_float2(-3.f, -3.f));
-    s.ax = __ffma2_rn(mri3, dx, s.ax);
-    s.ay = __ffma2_rn(mri3, dy, s.ay);
-    s.az = __ffma2_rn(mri3, dz, s.az);
-    s.jx = __ffma2_rn(mri3, __ffma2_rn(al, dx, dvx), s.jx);
-    s.jy = __ffma2_rn(mri3, __ffma2_rn(al, dy, dvy), s.jy);
-    s.jz = __ffma2_rn(mri3, __ffma2_rn(al, dz, dvz), s.jz);
+__device__ __forceinline__ float2 bc(float a) { return make_float2(a, a); }
+
+// The packed pair arithmetic, two j-particles (the halves of each float2) against one i.
+//
+// Far/near split (what keeps the common path at 25 packed FP32 instructions per two pairs):
+//   * every pair first forms R from the HIGH words only, R_hi = xh_j - xh_i, and r_hi^2;
+//   * if r_hi^2 >= hfar2 for both halves in every lane of the warp, the pair is FAR: it cannot be a neighbour
+//     (hfar2 >= r_s^2 (1 + 2^-10)) and R_hi is used as R.  The omitted low words change r by at most
+//     2^-24 (2 sqrt(3) X / r + 1) relative, X = max |x_i| component; hfar2 >= (X/4)^2 bounds that by 8.9e-7
+//     (worst case);
+//   * otherwise the warp takes the NEAR path: R = R_hi + (xl_j - xl_i) ("pseudo double precision for the
+//     coordinate differences", footnote at PAPER.md:154), r^2 is recomputed, the neighbour test
+//     eq. (2)/(11) is made on it, neighbours are appended to the list and masked by r^2 := +inf, so that
+//     rsqrt and rcp return 0 ("rinv1 = 0.f", Listing B2) and the pair adds nothing.
+struct PairGeom {
+    float2 dx, dy, dz, r2;
+};
+
+__device__ __forceinline__ void geom_hi(const float4& q0, const float4& q1, const IState& I, PairGeom& g) {
+    g.dx = __fadd2_rn(make_float2(q0.x, q0.y), bc(I.nxh));
+    g.dy = __fadd2_rn(make_float2(q0.z, q0.w), bc(I.nyh));
+    g.dz = __fadd2_rn(make_float2(q1.x, q1.y), bc(I.nzh));
+    g.r2 = __ffma2_rn(g.dz, g.dz, __ffma2_rn(g.dy, g.dy, __fmul2_rn(g.dx, g.dx)));
 }
 
-__device__ __forceinline__ void append(IState& I, int32_t j, bool nb, int32_t cap) {
+__device__ __forceinline__ void geom_lo(const float2& xl, const float4& q4, const IState& I, PairGeom& g) {
+    g.dx = __fadd2_rn(g.dx, __fadd2_rn(xl, bc(I.nxl)));
+    g.dy = __fadd2_rn(g.dy, __fadd2_rn(make_float2(q4.x, q4.y), bc(I.nyl)));
+    g.dz = __fadd2_rn(g.dz, __fadd2_rn(make_float2(q4.z, q4.w), bc(I.nzl)));
+    g.r2 = __ffma2_rn(g.dz, g.dz, __ffma2_rn(g.dy, g.dy, __fmul2_rn(g.dx, g.dx)));
+}
+
+// eq. (9), (10) for the two pairs: 3 FADD2 (V), 3 (R.V), 2 (m/r^3), 2 (alpha), 9 FFMA2 (sums); 2 MUFU.RSQ + 2 MUFU.RCP.
+__device__ __forceinline__ void pair_sum(const float4& q1, const float4& q2, const float2& vz, const IState& I,
+                                         const PairGeom& g, Accum& s) {
+    const float2 dvx = __fadd2_rn(make_float2(q2.x, q2.y), bc(I.nvx));
+    const float2 dvy = __fadd2_rn(make_float2(q2.z, q2.w), bc(I.nvy));
+    const float2 dvz = __fadd2_rn(vz, bc(I.nvz));
+    const float2 rv = __ffma2_rn(g.dz, dvz, __ffma2_rn(g.dy, dvy, __fmul2_rn(g.dx, dvx)));
+    const float2 ri = make_float2(rsqrt_approx(g.r2.x), rsqrt_approx(g.r2.y));
+    const float2 ri2 = make_float2(rcp_approx(g.r2.x), rcp_approx(g.r2.y));
+    const float2 mri3 = __fmul2_rn(__fmul2_rn(make_float2(q1.z, q1.w), ri), ri2);
+    const float2 al = __fmul2_rn(__fmul2_rn(rv, ri2), bc(-3.f));
+    s.ax = __ffma2_rn(mri3, g.dx, s.ax);
+    s.ay = __ffma2_rn(mri3, g.dy, s.ay);
+    s.az = __ffma2_rn(mri3, g.dz, s.az);
+    s.jx = __ffma2_rn(mri3, __ffma2_rn(al, g.dx, dvx), s.jx);
+    s.jy = __ffma2_rn(mri3, __ffma2_rn(al, g.dy, dvy), s.jy);
+    s.jz = __ffma2_rn(mri3, __ffma2_rn(al, g.dz, dvz), s.jz);
+}
+
+// S4: "the index j is written to the neighbour list in the memory".  A main-path row is owned by
+// one thread for the whole j-range: private counter, entries land in ascending j.  A j-split row is shared by
+// the CTAs of its chunks: a slot is reserved with an atomic on the row's final count (reduce_gather_kernel puts
+// the row in order afterwards).  The atomic's return value takes an L2 round trip, so the store that needs it
+// is DEFERRED to the thread's next append (or the end of the chunk): the warp never waits for it in the j-loop.
+// Entries past cap are dropped, the count keeps counting (reading R7).
+__device__ __forceinline__ void flush_pending(IState& I, int32_t cap) {
+    if (I.pend_j >= 0 && I.pend_pos < cap) I.list[I.pend_pos] = I.pend_j;
+    I.pend_j = -1;
+}
+__device__ __forceinline__ void append(IState& I, int32_t j, bool nb, int32_t cap, int32_t* shared_count) {
     if (nb && j != I.self && j < I.nlim) {
-        if (I.cnt < cap) I.list[I.cnt] = j;  // entries past cap are dropped, the count keeps counting (R7)
-        ++I.cnt;
+        if (shared_count) {
+            flush_pending(I, cap);
+            I.pend_pos = atomicAdd(shared_count, 1);
+            I.pend_j = j;
+        } else {
+            if (I.cnt < cap) I.list[I.cnt] = j;
+            ++I.cnt;
+        }
     }
 }
 
@@ -162,10 +209,17 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + kStages * kTileBytes);
 
     const int tid = threadIdx.x;
-    const int chunk = blockIdx.y;
-    const int t_begin = chunk * a.tiles_per_chunk;
-    const int t_end = min(t_begin + a.tiles_per_chunk, a.n_tiles);
+    const bool split = (int)blockIdx.x >= a.main_blocks;
+    int row_block = blockIdx.x, chunk = 0, t_begin = 0, t_end = a.n_tiles;
+    if (split) {
+        const int t = blockIdx.x - a.main_blocks;
+        row_block = a.main_blocks + t / a.n_chunks;
+        chunk = t % a.n_chunks;
+        t_begin = chunk * a.tiles_per_chunk;
+        t_end = min(t_begin + a.tiles_per_chunk, a.n_tiles);
+    }
     const int n_t = t_end - t_begin;
+    const int64_t tail_row0 = (int64_t)a.main_blocks * kRows;
 
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
@@ -184,30 +238,31 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
     int64_t rows[IPT];
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
-        const int64_t row = (int64_t)blockIdx.x * kRows + u * kThreads + tid;
+        const int64_t row = (int64_t)row_block * kRows + u * kThreads + tid;
         rows[u] = row;
         const bool live = row < a.n_i;
         const int32_t i = live ? a.i_idx[row] : 0;
         const float* rec = reinterpret_cast<const float*>(a.packed + (size_t)(i >> 1) * kQuadsPerPair);
         const int h = i & 1;
         const float xh = rec[0 + h], yh = rec[2 + h], zh = rec[4 + h];
-        const float xl = rec[8 + h], yl = rec[10 + h], zl = rec[12 + h];
-        const float vx = rec[14 + h], vy = rec[16 + h], vz = rec[18 + h];
-        I[u].nxh = make_float2(-xh, -xh); I[u].nyh = make_float2(-yh, -yh); I[u].nzh = make_float2(-zh, -zh);
-        I[u].nxl = make_float2(-xl, -xl); I[u].nyl = make_float2(-yl, -yl); I[u].nzl = make_float2(-zl, -zl);
-        I[u].nvx = make_float2(-vx, -vx); I[u].nvy = make_float2(-vy, -vy); I[u].nvz = make_float2(-vz, -vz);
+        const float vx = rec[8 + h], vy = rec[10 + h], vz = rec[12 + h];
+        const float xl = rec[14 + h], yl = rec[16 + h], zl = rec[18 + h];
+        I[u].nxh = -xh; I[u].nyh = -yh; I[u].nzh = -zh;
+        I[u].nxl = -xl; I[u].nyl = -yl; I[u].nzl = -zl;
+        I[u].nvx = -vx; I[u].nvy = -vy; I[u].nvz = -vz;
         const double rs = live ? a.r_s[row] : 0.0;
         const float h2 = __double2float_rn(rs * rs);
         // dead rows (past n_i) get h2 < 0: nothing is ever a neighbour, nothing is written
         I[u].h2 = live ? fmaxf(h2, 1.17549435e-38f) : -1.f;
+        // far threshold: beyond r_s with a 2^-10 margin, and beyond X/4 (X = largest |coordinate| of i), see above
+        const float xmax = fmaxf(fabsf(xh), fmaxf(fabsf(yh), fabsf(zh)));
+        I[u].hfar2 = live ? fmaxf(I[u].h2 * 1.0009765625f, 0.0625f * xmax * xmax) : -1.f;
         I[u].self = i;
         I[u].nlim = (live && h2 >= 1.17549435e-38f) ? a.n : 0;
         I[u].cnt = 0;
-        if (a.n_chunks == 1) {
-            I[u].list = a.nbr_list + (size_t)row * a.cap;
-        } else {
-            I[u].list = a.part_list + ((size_t)row * a.n_chunks + chunk) * a.cap;
-        }
+        I[u].pend_j = -1;
+        I[u].pend_pos = 0;
+        I[u].list = a.nbr_list + (size_t)row * a.cap;
         accum_zero(s[u]);
 #pragma unroll
         for (int c = 0; c < 6; ++c) sum[u][c] = 0.0;
@@ -226,23 +281,33 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         const int32_t jbase = (t_begin + lt) * JT;
 #pragma unroll 2
         for (int p = 0; p < JT / 2; ++p) {
-            const float4 q0 = tp[p * 5 + 0], q1 = tp[p * 5 + 1], q2 = tp[p * 5 + 2], q3 = tp[p * 5 + 3],
-                         q4 = tp[p * 5 + 4];
-            bool nb0[IPT], nb1[IPT];
-            bool any = false;
+            const float4 q0 = tp[p * 5 + 0], q1 = tp[p * 5 + 1], q2 = tp[p * 5 + 2];
+            const float2 vz = *reinterpret_cast<const float2*>(tp + p * 5 + 3);
+            PairGeom g[IPT];
+            bool near = false;
 #pragma unroll
             for (int u = 0; u < IPT; ++u) {
-                pair_step(q0, q1, q2, q3, q4, I[u], s[u], nb0[u], nb1[u]);
-                any = any || nb0[u] || nb1[u];
+                geom_hi(q0, q1, I[u], g[u]);
+                near = near || fminf(g[u].r2.x, g[u].r2.y) < I[u].hfar2;
             }
-            if (__any_sync(0xffffffffu, any)) {  // S4: rare path, warp-uniform branch
+            if (__any_sync(0xffffffffu, near)) {  // NEAR path (S4 lives here): rare, warp-uniform branch
+                const float2 xl = *(reinterpret_cast<const float2*>(tp + p * 5 + 3) + 1);
+                const float4 q4 = tp[p * 5 + 4];
                 const int32_t j = jbase + 2 * p;
 #pragma unroll
                 for (int u = 0; u < IPT; ++u) {
-                    append(I[u], j, nb0[u], a.cap);
-                    append(I[u], j + 1, nb1[u], a.cap);
+                    geom_lo(xl, q4, I[u], g[u]);
+                    const bool nb0 = g[u].r2.x < I[u].h2;  // eq. (2)/(11): neighbour iff r^2 < r_s^2
+                    const bool nb1 = g[u].r2.y < I[u].h2;
+                    int32_t* shared_count = split ? a.nbr_count + rows[u] : nullptr;
+                    append(I[u], j, nb0, a.cap, shared_count);
+                    append(I[u], j + 1, nb1, a.cap, shared_count);
+                    if (nb0) g[u].r2.x = __int_as_float(0x7f800000);
+                    if (nb1) g[u].r2.y = __int_as_float(0x7f800000);
                 }
             }
+#pragma unroll
+            for (int u = 0; u < IPT; ++u) pair_sum(q1, q2, vz, I[u], g[u], s[u]);
         }
         // ---- S6: flush the tile's fp32 partial sums into the fp64 running sums
 #pragma unroll
@@ -263,7 +328,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
     for (int u = 0; u < IPT; ++u) {
         const int64_t row = rows[u];
         if (row >= a.n_i) continue;
-        if (a.n_chunks == 1) {
+        if (!split) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 a.acc[row * 3 + c] = sum[u][c];
@@ -272,10 +337,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
             a.nbr_count[row] = I[u].cnt;
             if (I[u].cnt > a.cap) atomicAdd(a.n_overflow, 1);
         } else {
-            double* ps = a.part_sum + ((size_t)row * a.n_chunks + chunk) * 6;
+            flush_pending(I[u], a.cap);
+            const size_t pi = (size_t)(row - tail_row0) * a.n_chunks + chunk;
+            double* ps = a.part_sum + pi * 6;
 #pragma unroll
             for (int c = 0; c < 6; ++c) ps[c] = sum[u][c];
-            a.part_cnt[(size_t)row * a.n_chunks + chunk] = I[u].cnt;
         }
     }
 }

@@ -1,27 +1,30 @@
-// gather.cuh -- S5: cross-CTA partial-sum reduction and neighbour-list gathering for the j-split path.
+// gather.cuh -- S5: cross-CTA partial-sum reduction and neighbour-list gathering for the j-split rows.
 //
 // "partial forces and partial neighbour lists ... are distributed for multiple thread-blocks ... we prepared
 // kernels for force reduction and list gathering ... Partial forces are summed and sparsely scattered partial
-// lists are serialized to a linear array".  Here: one warp per row; lanes run over the
-// row's j-chunks.  Sums: fp64, lane-strided then a fixed xor-shuffle tree, so the result is deterministic.
-// Lists: the chunks were scanned in ascending j, so concatenating them in chunk order gives an ascending
-// list; a warp ballot finds the (few) non-empty chunks, a shuffle scan of the chunk counts gives each its
-// offset, and the entries are copied with coalesced lane-parallel loads/stores.
+// lists are serialized to a linear array".  Here: one warp per j-split row.
+//   Sums: fp64; lanes stride over the row's j-chunks, then a fixed xor-shuffle tree: deterministic.
+//   Lists: the chunks' CTAs appended their neighbours to the row's final list in arrival order (atomic slot
+//   counter, force.cuh).  Each chunk covers a contiguous j-range and its entries arrive in ascending j, so the
+//   ascending order is restored by a stable counting sort on the chunk number, done by the warp: a
+//   match_any/popc vote groups the lanes of each 32-entry block by chunk (the warp-vote compaction idiom,
+//   ballot + popc), per-chunk counters live in shared memory, a shuffle scan turns them into offsets, and a
+//   second pass writes every entry to offset[chunk] + its rank among earlier entries of the same chunk.  O(count + S).
 #pragma once
 #include "nbreg_common.cuh"
 
 namespace nbreg {
 
 struct GatherArgs {
+    int32_t row0;              // first j-split row (rows below were written directly by the force kernel)
     int32_t n_i;
     int32_t n_chunks;
+    int32_t chunk_j;           // j-particles per chunk (tiles_per_chunk * j-tile)
     int32_t cap;
-    const double* part_sum;    // [rows][S][6]
-    const int32_t* part_cnt;   // [rows][S]
-    const int32_t* part_list;  // [rows][S][cap]
+    const double* part_sum;    // [split rows][S][6]
     double* acc;
     double* jerk;
-    int32_t* nbr_count;
+    const int32_t* nbr_count;  // final (true) counts, complete when this kernel starts
     int32_t* nbr_list;
     int32_t* n_overflow;
 };
@@ -29,11 +32,14 @@ struct GatherArgs {
 constexpr int kGatherWarps = 4;
 
 __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(GatherArgs a) {
+    extern __shared__ int32_t stage_all[];  // kGatherWarps x (cap + S)
     const int lane = threadIdx.x & 31;
-    const int64_t row = (int64_t)blockIdx.x * kGatherWarps + (threadIdx.x >> 5);
+    const int warp = threadIdx.x >> 5;
+    const int64_t prow = (int64_t)blockIdx.x * kGatherWarps + warp;  // row among the split rows
+    const int64_t row = a.row0 + prow;
     if (row >= a.n_i) return;  // warp-uniform
     const int S = a.n_chunks;
-    const size_t rbase = (size_t)row * S;
+    const size_t rbase = (size_t)prow * S;
 
     // ---- partial sums (fixed order: chunk = lane, lane + 32, ...; then xor tree 16, 8, 4, 2, 1)
     double s[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
@@ -52,36 +58,51 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
         a.jerk[row * 3 + lane] = (lane == 0) ? s[3] : (lane == 1) ? s[4] : s[5];
     }
 
-    // ---- lists: compact the non-empty chunks into the row, ascending j
+    // ---- list: stable counting sort of the stored entries by chunk number
+    const int32_t cnt = a.nbr_count[row];  // true count, may exceed cap
+    const int32_t stored = min(cnt, a.cap);
     int32_t* out = a.nbr_list + (size_t)row * a.cap;
-    int32_t base = 0;
-    for (int c0 = 0; c0 < S; c0 += 32) {
+    int32_t* stage = stage_all + (size_t)warp * (a.cap + S);
+    int32_t* bin = stage + a.cap;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    for (int32_t e = lane; e < stored; e += 32) stage[e] = out[e];
+    for (int c = lane; c < S; c += 32) bin[c] = 0;
+    __syncwarp();
+    for (int32_t e0 = 0; e0 < stored; e0 += 32) {  // pass 1: entries per chunk
+        const int32_t e = e0 + lane;
+        const bool valid = e < stored;
+        const int32_t c = valid ? stage[e] / a.chunk_j : S;
+        const uint32_t peers = __match_any_sync(0xffffffffu, c);
+        if (valid && (peers & lt_mask) == 0) bin[c] += __popc(peers);  // one leader per chunk in this block
+        __syncwarp();
+    }
+    int32_t carry = 0;
+    for (int c0 = 0; c0 < S; c0 += 32) {  // exclusive scan of the counters -> first slot of each chunk
         const int c = c0 + lane;
-        const int32_t cn = (c < S) ? a.part_cnt[rbase + c] : 0;
-        int32_t incl = cn;  // inclusive scan over lanes
+        const int32_t x = (c < S) ? bin[c] : 0;
+        int32_t incl = x;
 #pragma unroll
         for (int off = 1; off < 32; off <<= 1) {
-            const int32_t v = __shfl_up_sync(0xffffffffu, incl, off);
-            if (lane >= off) incl += v;
+            const int32_t y = __shfl_up_sync(0xffffffffu, incl, off);
+            if (lane >= off) incl += y;
         }
-        const int32_t excl = incl - cn;
-        uint32_t nonempty = __ballot_sync(0xffffffffu, cn > 0);
-        while (nonempty) {  // popc(nonempty) iterations, warp-uniform
-            const int src = __ffs(nonempty) - 1;
-            nonempty &= nonempty - 1;
-            const int32_t n_src = min(__shfl_sync(0xffffffffu, cn, src), a.cap);  // a partial list holds <= cap
-            const int32_t off = base + __shfl_sync(0xffffffffu, excl, src);
-            const int32_t* in = a.part_list + (rbase + c0 + src) * a.cap;
-            for (int32_t e = lane; e < n_src; e += 32) {
-                if (off + e < a.cap) out[off + e] = in[e];
-            }
-        }
-        base += __shfl_sync(0xffffffffu, incl, 31);
+        if (c < S) bin[c] = carry + incl - x;
+        carry += __shfl_sync(0xffffffffu, incl, 31);
     }
-    if (lane == 0) {
-        a.nbr_count[row] = base;  // true count, may exceed cap
-        if (base > a.cap) atomicAdd(a.n_overflow, 1);
+    __syncwarp();
+    for (int32_t e0 = 0; e0 < stored; e0 += 32) {  // pass 2: scatter, arrival order kept within a chunk
+        const int32_t e = e0 + lane;
+        const bool valid = e < stored;
+        const int32_t v = valid ? stage[e] : 0;
+        const int32_t c = valid ? v / a.chunk_j : S;
+        const uint32_t peers = __match_any_sync(0xffffffffu, c);
+        const int32_t before = __popc(peers & lt_mask);
+        if (valid) out[bin[c] + before] = v;
+        __syncwarp();
+        if (valid && before == 0) bin[c] += __popc(peers);
+        __syncwarp();
     }
+    if (lane == 0 && cnt > a.cap) atomicAdd(a.n_overflow, 1);
 }
 
 }  // namespace nbreg

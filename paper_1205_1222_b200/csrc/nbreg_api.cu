@@ -3,7 +3,10 @@
 #include "../../include/nbreg.h"
 
 #include <cstdio>
+#include <algorithm>
+#include <cmath>
 #include <cstring>
+#include <utility>
 #include <new>
 
 #include "force.cuh"
@@ -12,6 +15,12 @@
 #include "predict.cuh"
 
 using namespace nbreg;
+
+// Resident 256-thread CTAs per SM the one-i-per-thread force kernels are compiled for (register cap
+// 65536 / (256 * NBREG_CTAS256)); smaller CTA shapes scale it so that the warps per SM stay the same.
+#ifndef NBREG_CTAS256
+#define NBREG_CTAS256 3
+#endif
 
 namespace {
 
@@ -27,33 +36,46 @@ int cuda_fail(cudaError_t e, const char* what) {
         if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
     } while (0)
 
-// Launch plan of the force kernel: CTA shape and j-split.
+// CTA shapes of the force kernel.  All one-i-per-thread shapes keep the same number of resident warps per SM
+// (8 * NBREG_CTAS256); the 512-row shape (two i per thread) is only used when asked for.
+constexpr int kNumShapes = 5;
+struct Shape {
+    int rows, ipt, warps, jt;
+};
+constexpr Shape kShapes[kNumShapes] = {{256, 1, 8, 256}, {128, 1, 4, 128}, {64, 1, 2, 128}, {32, 1, 1, 64},
+                                       {512, 2, 8, 256}};
+
+// Launch plan of the force kernel: CTA shape, how many row blocks run the whole j-range in one CTA ("main"),
+// and the j-split of the remaining ("tail") row blocks.
 struct Plan {
-    int rows_per_cta;  // IB = 32 * warps * ipt
-    int ipt;
-    int warps;
-    int jt;            // j per shared-memory tile
-    int n_chunks;      // S
+    int shape;          // index into kShapes
+    int n_tiles;        // j-tiles of kShapes[shape].jt covering n_pad
+    int n_blocks;       // row blocks
+    int main_blocks;    // row blocks handled by one CTA each
+    int n_chunks;       // S: j-chunks per tail row block (1 = no tail: main_blocks == n_blocks)
     int tiles_per_chunk;
-    int n_tiles;
-    int grid_x;
+    int grid;           // CTAs
+    double cost;        // model cost in units of (one j against one CTA's rows)
 };
 
 struct WorkspaceLayout {
     size_t packed_off, packed_bytes;
     size_t psum_off, psum_bytes;
-    size_t pcnt_off, pcnt_bytes;
-    size_t plist_off, plist_bytes;
+    int64_t row_chunk_limit;  // (row, j-chunk) slots of partial sums
     size_t total;
 };
 
+// The j-split workspace holds 6 doubles per (row, chunk): enough slots for 64 chunks per row of the largest
+// block, at least 131072 (small blocks are split hundreds of ways), at most 2M (96 MB).
+int64_t row_chunk_slots(int64_t n_i_max) {
+    return std::min<int64_t>(std::max<int64_t>(64 * n_i_max, 131072), 2097152);
+}
+
 WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
     WorkspaceLayout w{};
+    (void)cap;
     const int64_t n_pad = round_up(n_max, kJPad);
-    // rows x chunks of the j-split path never exceed kRowChunkLimit (make_plan), nor is the path taken for
-    // blocks so large that one chunk per row suffices
-    const int64_t rc = kRowChunkLimit;
-    (void)n_i_max;
+    w.row_chunk_limit = row_chunk_slots(n_i_max);
     size_t off = 0;
     auto place = [&](size_t bytes, size_t& o, size_t& b) {
         o = off;
@@ -61,9 +83,7 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
         off += (size_t)round_up((int64_t)bytes, 256);
     };
     place((size_t)n_pad * kBytesPerJ, w.packed_off, w.packed_bytes);
-    place((size_t)rc * 6 * sizeof(double), w.psum_off, w.psum_bytes);
-    place((size_t)rc * sizeof(int32_t), w.pcnt_off, w.pcnt_bytes);
-    place((size_t)rc * (size_t)cap * sizeof(int32_t), w.plist_off, w.plist_bytes);
+    place((size_t)w.row_chunk_limit * 6 * sizeof(double), w.psum_off, w.psum_bytes);
     w.total = off;
     return w;
 }
@@ -73,6 +93,7 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
 struct nb_ctx {
     int device = 0;
     int num_sms = 0;
+    int ctas_per_sm[kNumShapes] = {0, 0, 0, 0, 0};  // resident CTAs per SM of each force-kernel shape
     int64_t n_max = 0, n_i_max = 0;
     int32_t cap = 0;
     unsigned char* ws = nullptr;
@@ -84,7 +105,7 @@ struct nb_ctx {
     bool predicted = false;
     double t_pred = 0.0;
     // options
-    int64_t opt_j_split = 0, opt_i_block = 0, opt_warp_target = 0;
+    int64_t opt_j_split = 0, opt_i_block = 0;
     // last launch
     int64_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     // host path: device mirrors owned by the context
@@ -95,63 +116,134 @@ struct nb_ctx {
 
 namespace {
 
-Plan make_plan(const nb_ctx* c, int32_t n_i) {
+// Cost model behind the plan, in units of "one j against the rows of one CTA".  All
+// resident warps share an SM evenly, so a CTA needs a time proportional to the j it covers, plus a prologue worth
+// ~kPrologueJ j, whatever its shape.  Row blocks that fill whole waves of CTA slots run the full j-range in one
+// CTA and write their outputs directly.  The remaining ("tail") blocks -- all blocks of a small active block --
+// are split S ways along j.  Measured on B200 (profiles/, planner calibration): G equal CTAs
+// of duration t on `slots` slots take about w t + 0.2 t, w between G / slots and its ceiling; the last term is the
+// ragged end, which is why several waves of short CTAs beat one wave of long ones.
+constexpr double kPrologueJ = 48.0;
+constexpr double kRaggedEnd = 0.2;
+
+struct Machine {
+    int64_t n;        // j-particles
+    int64_t row_chunk_limit;
+    int num_sms;
+    int ctas_per_sm[kNumShapes];
+};
+
+Plan plan_for_shape(const Machine* c, int32_t n_i, int shape, int64_t force_split) {
+    const Shape& sh = kShapes[shape];
     Plan p{};
+    p.shape = shape;
     const int64_t n_pad = round_up(c->n, kJPad);
+    p.n_tiles = (int)(n_pad / sh.jt);
+    p.n_blocks = (int)((n_i + sh.rows - 1) / sh.rows);
     const int64_t sms = c->num_sms > 0 ? c->num_sms : 148;
-    const int64_t min_ctas = 6 * sms;  // enough CTAs for the hardware scheduler to balance the SMs
-    int ib;
-    if (c->opt_i_block) {
-        ib = (int)c->opt_i_block;
-    } else if (n_i >= 256 * min_ctas) {
-        ib = 256;
-    } else if (n_i >= 128 * min_ctas) {
-        ib = 128;
-    } else if (n_i >= 64 * min_ctas) {
-        ib = 64;
+    const int64_t slots = sms * (c->ctas_per_sm[shape] > 0 ? c->ctas_per_sm[shape] : 1);
+    const double t_full = kPrologueJ + (double)n_pad;
+    auto chunking = [&](int64_t S) {  // tiles per chunk and the resulting number of non-empty chunks
+        const int tpc = (int)((p.n_tiles + S - 1) / S);
+        return std::pair<int, int>(tpc, (p.n_tiles + tpc - 1) / tpc);
+    };
+    auto tail_cost = [&](int64_t tail, const std::pair<int, int>& ch) {
+        const double t = kPrologueJ + (double)ch.first * sh.jt;
+        const double waves = (double)(tail * ch.second) / (double)slots;
+        // few waves run almost in lockstep (the count rounds up), many waves overlap freely
+        const double eff_waves = std::max(1.0, 0.5 * std::ceil(waves) + 0.5 * waves);
+        return eff_waves * t + kRaggedEnd * t;
+    };
+    int64_t tail = p.n_blocks, S = 1;
+    if (force_split > 0) {
+        S = force_split;
     } else {
-        ib = 32;
+        tail = p.n_blocks % slots;
+        if (tail > 0) {
+            int64_t s_max = std::min<int64_t>(p.n_tiles, c->row_chunk_limit / (tail * sh.rows));
+            s_max = std::max<int64_t>(1, std::min<int64_t>(s_max, kMaxChunks));
+            double best = 1e300;
+            int last_chunks = 0;
+            for (int64_t s = 1; s <= s_max; ++s) {
+                const auto ch = chunking(s);
+                if (ch.second == last_chunks) continue;  // same chunking as a smaller s
+                last_chunks = ch.second;
+                // an unsplit tail (s = 1) is one more full-length wave
+                const double cost = (ch.second == 1) ? t_full : tail_cost(tail, ch);
+                if (cost < best) {
+                    best = cost;
+                    S = s;
+                }
+            }
+        }
     }
-    switch (ib) {
-        case 32: p.ipt = 1; p.warps = 1; p.jt = 64; break;
-        case 64: p.ipt = 1; p.warps = 2; p.jt = 128; break;
-        case 128: p.ipt = 1; p.warps = 4; p.jt = 128; break;
-        case 256: p.ipt = 1; p.warps = 8; p.jt = 256; break;
-        default: p.ipt = 2; p.warps = 8; p.jt = 256; ib = 512; break;
-    }
-    p.rows_per_cta = ib;
-    p.grid_x = (int)((n_i + ib - 1) / ib);
-    p.n_tiles = (int)(n_pad / p.jt);
-    // j-split: when the block has too few warps to fill the machine, split the j-range
-    const int64_t warps_total = (n_i + 31) / 32;
-    const int64_t warp_target = c->opt_warp_target ? c->opt_warp_target : 16 * sms;
-    int64_t S = 1;
-    if (c->opt_j_split) {
-        S = c->opt_j_split;
-    } else if (warps_total < warp_target) {
-        S = (warp_target + warps_total - 1) / warps_total;
-    }
-    const int64_t rows_pad = (int64_t)p.grid_x * ib;
-    if (S > 1 && rows_pad * S > kRowChunkLimit) S = kRowChunkLimit / rows_pad;
     if (S > p.n_tiles) S = p.n_tiles;
-    if (S < 1) S = 1;
-    p.tiles_per_chunk = (int)((p.n_tiles + S - 1) / S);
-    p.n_chunks = (p.n_tiles + p.tiles_per_chunk - 1) / p.tiles_per_chunk;
+    if (S > kMaxChunks) S = kMaxChunks;
+    if (S > 1 && tail * sh.rows * S > c->row_chunk_limit) S = std::max<int64_t>(1, c->row_chunk_limit / (tail * sh.rows));
+    const auto ch = chunking(S);
+    p.tiles_per_chunk = ch.first;
+    p.n_chunks = ch.second;
+    if (p.n_chunks <= 1) {
+        p.n_chunks = 1;
+        tail = 0;
+    }
+    p.main_blocks = (int)(p.n_blocks - tail);
+    p.grid = (int)(p.main_blocks + tail * p.n_chunks);
+    const double main_waves = (double)((p.main_blocks + slots - 1) / slots);
+    p.cost = main_waves * t_full + (tail ? tail_cost(tail, ch) : 0.0);
     return p;
 }
 
+Plan make_plan(const Machine* c, int32_t n_i, int64_t opt_i_block, int64_t opt_j_split) {
+    if (opt_i_block) {
+        int shape = 0;
+        for (int k = 0; k < kNumShapes; ++k)
+            if (kShapes[k].rows == opt_i_block) shape = k;
+        return plan_for_shape(c, n_i, shape, opt_j_split);
+    }
+    // smaller CTAs pay a little more for staging the j-tiles (fewer warps share one bulk copy)
+    const double penalty[4] = {1.0, 1.02, 1.04, 1.06};
+    Plan best{};
+    double best_cost = 1e300;
+    for (int k = 0; k < 4; ++k) {
+        const Plan p = plan_for_shape(c, n_i, k, opt_j_split);
+        if (p.cost * penalty[k] < best_cost) {
+            best_cost = p.cost * penalty[k];
+            best = p;
+        }
+    }
+    return best;
+}
+
 template <int IPT, int WARPS, int JT, int MINB>
-int launch_force(nb_ctx* c, const Plan& p, const ForceArgs& fa, cudaStream_t st) {
+int query_force(int* per_sm) {
     auto kern = force_kernel<IPT, WARPS, JT, MINB>;
     const size_t smem = 2 * (size_t)JT * kBytesPerJ + 2 * sizeof(uint64_t);
     NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int per_sm = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, WARPS * 32, smem);
-    c->info[7] = per_sm;
-    dim3 grid(p.grid_x, p.n_chunks);
-    kern<<<grid, WARPS * 32, smem, st>>>(fa);
+    NB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, WARPS * 32, smem));
+    return NB_OK;
+}
+
+template <int IPT, int WARPS, int JT, int MINB>
+int launch_force(const Plan& p, const ForceArgs& fa, cudaStream_t st) {
+    const size_t smem = 2 * (size_t)JT * kBytesPerJ + 2 * sizeof(uint64_t);
+    force_kernel<IPT, WARPS, JT, MINB><<<p.grid, WARPS * 32, smem, st>>>(fa);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
+}
+
+// one switch for both: keeps the template arguments of query and launch in one place
+int force_dispatch(int shape, int* per_sm, const Plan* p, const ForceArgs* fa, cudaStream_t st) {
+#define NB_SHAPE(IPT, WARPS, JT, MINB) \
+    (per_sm ? query_force<IPT, WARPS, JT, MINB>(per_sm) : launch_force<IPT, WARPS, JT, MINB>(*p, *fa, st))
+    switch (shape) {
+        case 0: return NB_SHAPE(1, 8, 256, NBREG_CTAS256);
+        case 1: return NB_SHAPE(1, 4, 128, 2 * NBREG_CTAS256);
+        case 2: return NB_SHAPE(1, 2, 128, 4 * NBREG_CTAS256);
+        case 3: return NB_SHAPE(1, 1, 64, 8 * NBREG_CTAS256);
+        default: return NB_SHAPE(2, 8, 256, 1);
+    }
+#undef NB_SHAPE
 }
 
 int run_predict(nb_ctx* c, double t, cudaStream_t st, double* xp_out, double* vp_out) {
@@ -195,7 +287,9 @@ const char* nb_strerror(int code) {
 }
 
 size_t nb_workspace_bytes(int64_t n_max, int64_t n_i_max, int32_t nbr_cap) {
-    if (n_max < 1 || n_i_max < 0 || nbr_cap < 1 || n_max > 0x7fffff00LL || n_i_max > 0x7fffffffLL) return 0;
+    if (n_max < 1 || n_i_max < 0 || nbr_cap < 1 || nbr_cap > kMaxNbrCap || n_max > 0x7fffff00LL ||
+        n_i_max > 0x7fffffffLL)
+        return 0;
     return layout(n_max, n_i_max, nbr_cap).total;
 }
 
@@ -215,6 +309,18 @@ int nb_create(nb_ctx** out, int device, int64_t n_max, int64_t n_i_max, int32_t 
     if (!c) return NB_E_NOMEM;
     c->device = device;
     cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
+    if (cudaFuncSetAttribute(reduce_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)((size_t)kGatherWarps * (nbr_cap + kMaxChunks) * sizeof(int32_t))) != cudaSuccess) {
+        delete c;
+        return cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(reduce_gather_kernel)");
+    }
+    for (int k = 0; k < kNumShapes; ++k) {
+        const int rc = force_dispatch(k, &c->ctas_per_sm[k], nullptr, nullptr, nullptr);
+        if (rc != NB_OK) {
+            delete c;
+            return rc;
+        }
+    }
     c->n_max = n_max;
     c->n_i_max = n_i_max;
     c->cap = nbr_cap;
@@ -296,11 +402,17 @@ int nb_regular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const double*
         c->info[5] = launches;
         return NB_OK;
     }
-    const Plan p = make_plan(c, n_i);
+    Machine mach{};
+    mach.n = c->n;
+    mach.row_chunk_limit = c->lay.row_chunk_limit;
+    mach.num_sms = c->num_sms;
+    for (int k = 0; k < kNumShapes; ++k) mach.ctas_per_sm[k] = c->ctas_per_sm[k];
+    const Plan p = make_plan(&mach, n_i, c->opt_i_block, c->opt_j_split);
     ForceArgs fa{};
     fa.packed = reinterpret_cast<const float4*>(c->ws + c->lay.packed_off);
     fa.n = (int32_t)c->n;
     fa.n_tiles = p.n_tiles;
+    fa.main_blocks = p.main_blocks;
     fa.tiles_per_chunk = p.tiles_per_chunk;
     fa.n_chunks = p.n_chunks;
     fa.n_i = n_i;
@@ -309,30 +421,29 @@ int nb_regular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const double*
     fa.r_s = r_s;
     fa.acc = acc; fa.jerk = jerk; fa.nbr_count = nbr_count; fa.nbr_list = nbr_list; fa.n_overflow = n_overflow;
     fa.part_sum = reinterpret_cast<double*>(c->ws + c->lay.psum_off);
-    fa.part_cnt = reinterpret_cast<int32_t*>(c->ws + c->lay.pcnt_off);
-    fa.part_list = reinterpret_cast<int32_t*>(c->ws + c->lay.plist_off);
-    int rc;
-    switch (p.rows_per_cta) {
-        case 32: rc = launch_force<1, 1, 64, 16>(c, p, fa, st); break;
-        case 64: rc = launch_force<1, 2, 128, 8>(c, p, fa, st); break;
-        case 128: rc = launch_force<1, 4, 128, 4>(c, p, fa, st); break;
-        case 256: rc = launch_force<1, 8, 256, 2>(c, p, fa, st); break;
-        default: rc = launch_force<2, 8, 256, 1>(c, p, fa, st); break;
-    }
+    const Shape& sh = kShapes[p.shape];
+    const int64_t row0 = (int64_t)p.main_blocks * sh.rows;
+    const bool has_split = p.n_chunks > 1 && row0 < n_i;
+    if (has_split)  // the split rows' CTAs reserve list slots with atomics on the final counts
+        NB_CUDA(cudaMemsetAsync(nbr_count + row0, 0, (size_t)(n_i - row0) * sizeof(int32_t), st));
+    int rc = force_dispatch(p.shape, nullptr, &p, &fa, st);
     if (rc != NB_OK) return rc;
     ++launches;
-    if (p.n_chunks > 1) {
+    if (has_split) {
         GatherArgs ga{};
-        ga.n_i = n_i; ga.n_chunks = p.n_chunks; ga.cap = c->cap;
-        ga.part_sum = fa.part_sum; ga.part_cnt = fa.part_cnt; ga.part_list = fa.part_list;
+        ga.row0 = (int32_t)row0; ga.n_i = n_i; ga.n_chunks = p.n_chunks; ga.cap = c->cap;
+        ga.chunk_j = p.tiles_per_chunk * sh.jt;
+        ga.part_sum = fa.part_sum;
         ga.acc = acc; ga.jerk = jerk; ga.nbr_count = nbr_count; ga.nbr_list = nbr_list; ga.n_overflow = n_overflow;
-        const unsigned blocks = (unsigned)((n_i + kGatherWarps - 1) / kGatherWarps);
-        reduce_gather_kernel<<<blocks, kGatherWarps * 32, 0, st>>>(ga);
+        const unsigned blocks = (unsigned)((n_i - row0 + kGatherWarps - 1) / kGatherWarps);
+        const size_t stage = (size_t)kGatherWarps * (c->cap + p.n_chunks) * sizeof(int32_t);
+        reduce_gather_kernel<<<blocks, kGatherWarps * 32, stage, st>>>(ga);
         NB_CUDA(cudaGetLastError());
         ++launches;
     }
-    c->info[0] = p.rows_per_cta; c->info[1] = p.ipt; c->info[2] = p.n_chunks; c->info[3] = p.grid_x;
-    c->info[4] = p.n_chunks; c->info[5] = launches; c->info[6] = p.jt;
+    c->info[0] = sh.rows; c->info[1] = sh.ipt; c->info[2] = p.n_chunks; c->info[3] = p.grid;
+    c->info[4] = p.n_blocks - p.main_blocks; c->info[5] = launches; c->info[6] = sh.jt;
+    c->info[7] = c->ctas_per_sm[p.shape];
     return NB_OK;
 }
 
@@ -405,11 +516,28 @@ int nb_set_option(nb_ctx* c, const char* key, int64_t value) {
         c->opt_i_block = value;
         return NB_OK;
     }
-    if (!strcmp(key, "warp_target")) {
-        c->opt_warp_target = value;
-        return NB_OK;
-    }
     return NB_E_INVAL;
+}
+
+int nb_plan(int64_t n, int32_t n_i, int32_t num_sms, const int32_t ctas_per_sm[5], int64_t i_block, int64_t j_split,
+            int64_t info[8]) {
+    if (n < 1 || n_i < 1 || num_sms < 1 || !ctas_per_sm || !info || j_split < 0) return NB_E_INVAL;
+    if (i_block != 0 && i_block != 32 && i_block != 64 && i_block != 128 && i_block != 256 && i_block != 512)
+        return NB_E_INVAL;
+    Machine mach{};
+    mach.n = n;
+    mach.row_chunk_limit = row_chunk_slots(n_i);
+    mach.num_sms = num_sms;
+    for (int k = 0; k < kNumShapes; ++k) {
+        if (ctas_per_sm[k] < 1) return NB_E_INVAL;
+        mach.ctas_per_sm[k] = ctas_per_sm[k];
+    }
+    const Plan p = make_plan(&mach, n_i, i_block, j_split);
+    const Shape& sh = kShapes[p.shape];
+    info[0] = sh.rows; info[1] = sh.ipt; info[2] = p.n_chunks; info[3] = p.grid;
+    info[4] = p.n_blocks - p.main_blocks; info[5] = p.tiles_per_chunk; info[6] = sh.jt;
+    info[7] = mach.ctas_per_sm[p.shape];
+    return NB_OK;
 }
 
 int nb_last_launch_info(const nb_ctx* c, int64_t info[8]) {

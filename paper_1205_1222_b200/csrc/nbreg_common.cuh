@@ -6,9 +6,10 @@
 // instruction operand pair directly:
 //     q0 = { xh0, xh1, yh0, yh1 }     position high words   (xh = fl32(x_p))
 //     q1 = { zh0, zh1, m0,  m1  }
-//     q2 = { xl0, xl1, yl0, yl1 }     position low words    (xl = fl32(x_p - xh): "two-float")
-//     q3 = { zl0, zl1, vx0, vx1 }
-//     q4 = { vy0, vy1, vz0, vz1 }     velocity, fl32
+//     q2 = { vx0, vx1, vy0, vy1 }     velocity, fl32
+//     q3 = { vz0, vz1, xl0, xl1 }     position low words    (xl = fl32(x_p - xh): "two-float")
+//     q4 = { yl0, yl1, zl0, zl1 }
+// The low words sit at the end of the record: the common (far-pair) path of the force kernel never loads them.
 // = 40 B per j.  The array is padded with massless dummies parked far away up to a multiple of kJPad.
 #pragma once
 #include <cuda_runtime.h>
@@ -20,7 +21,8 @@ constexpr int kQuadsPerPair = 5;       // float4 per packed j-pair
 constexpr int kBytesPerJ = 40;         // packed bytes per j-particle
 constexpr int kJPad = 256;             // packed array length is a multiple of this (largest j-tile)
 constexpr float kFarAway = 1.0e18f;    // coordinate of the massless padding particles
-constexpr int64_t kRowChunkLimit = 131072;  // max (rows x j-chunks) the j-split workspace holds
+constexpr int kMaxChunks = 2048;       // most j-chunks a row block is split into
+constexpr int kMaxNbrCap = 8192;       // nbr_cap limit: the gather kernel stages 4 rows of cap entries in shared memory
 
 __host__ __device__ inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 

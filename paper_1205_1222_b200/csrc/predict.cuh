@@ -90,9 +90,9 @@ __global__ void __launch_bounds__(256) predict_kernel(PredictArgs a) {
         float4* o = a.packed + kQuadsPerPair * p;
         o[0] = make_float4(xh[0], xh[3], xh[1], xh[4]);
         o[1] = make_float4(xh[2], xh[5], mf[0], mf[1]);
-        o[2] = make_float4(xl[0], xl[3], xl[1], xl[4]);
-        o[3] = make_float4(xl[2], xl[5], vf[0], vf[3]);
-        o[4] = make_float4(vf[1], vf[4], vf[2], vf[5]);
+        o[2] = make_float4(vf[0], vf[3], vf[1], vf[4]);
+        o[3] = make_float4(vf[2], vf[5], xl[0], xl[3]);
+        o[4] = make_float4(xl[1], xl[4], xl[2], xl[5]);
     }
 }
 

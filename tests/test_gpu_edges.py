@@ -46,6 +46,18 @@ def test_shapes_and_splits_agree_bitwise_on_lists_and_closely_on_sums(oracle):
         assert parity.relerr(g["acc"], ref["acc"]).max() < 5e-7
 
 
+@pytest.mark.parametrize("i_block", [32, 0])
+def test_main_blocks_plus_split_tail(oracle, i_block):
+    """More row blocks than CTA slots: whole waves run unsplit, the remaining blocks are j-split (atomic list
+    slots + rank sort in the gather kernel).  Rows are drawn with replacement so that N stays small."""
+    wl = _wl(oracle, 3001, 120001 if i_block else 250007, 24, 64)
+    gpu, info = run_gpu(wl, options={"i_block": i_block})
+    n_blocks = -(-wl.n_i // info["rows_per_cta"])
+    assert 0 < info["split_row_blocks"] < n_blocks and info["j_chunks"] > 1
+    assert info["ctas"] == n_blocks - info["split_row_blocks"] + info["split_row_blocks"] * info["j_chunks"]
+    _full_check(oracle, wl, gpu)
+
+
 def test_deterministic_repeat(oracle):
     wl = _wl(oracle, 5000, 300, 20, 64)
     a, _ = run_gpu(wl)
