@@ -29,6 +29,12 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 FLOPS_PER_PAIR = 60.0  # convention of BASELINE.json ("e.g. 60 for force+jerk"), SURVEY.md R13
+# FP32-pipe work the force kernel actually issues: 25 packed f32x2 instructions per TWO pairs on the common (far)
+# path = 25 of the SM's 128 FP32 lane-slots per pair.
+LANE_SLOTS_PER_PAIR = 25.0
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE force_kernel launch of the default workload, from the
+# committed capture profiles/r1_force_kernel_c5_ncu_full.md (ncu --set full); None for other workloads.
+FORCE_DRAM_BYTES_C5 = 529.45e6 + 665.25e6
 METRIC = "regular-force Ginteractions/s (acc+jerk+nbr list)"
 UNIT = "Gpairs/s"
 
@@ -81,6 +87,21 @@ class ClockSampler:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
                 "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def max_over_ranks(seconds: float, dist, device) -> float:
+    """Replicas only: every rank runs the same workload on its own GPU, no data-path
+    collective.  The job's time is the slowest rank's; this MAX all-reduce is the only communication."""
+    import torch
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(pairs_per_rank_step: int, steps: int, world: int, t_max_seconds: float) -> float:
+    """G pairs/s of the whole job: all ranks' pairs over the slowest rank's time."""
+    return world * pairs_per_rank_step * steps / t_max_seconds / 1e9
 
 
 def build_workload(config: int, n_i: int | None):
@@ -204,10 +225,8 @@ def run_gpu_arm(args):
     t_step = sum(e[0].elapsed_time(e[2]) for e in evs) / 1e3          # s, all K steps, device time
     t_pred = sum(e[0].elapsed_time(e[1]) for e in evs) / 1e3 / args.steps
     t_force = sum(e[1].elapsed_time(e[2]) for e in evs) / 1e3 / args.steps
-    tt = torch.tensor([t_step], dtype=torch.float64, device=dev)
-    if dist: dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_max = float(tt.item())
-    value = world * wl.pairs * args.steps / t_max / 1e9
+    t_max = max_over_ranks(t_step, dist, dev)
+    value = whole_job_rate(wl.pairs, args.steps, world, t_max)
     n_over = int(out["n_overflow"].item())
     mean_cnt = float(out["nbr_count"].double().mean().item())
 
@@ -232,11 +251,10 @@ def run_gpu_arm(args):
         for _ in range(ksteps):
             ctx.nb_regular_force_host(*h_in, h_idx, h_rs, s.t, h_out)  # synchronises internally
         te = time.perf_counter() - t0
-        te_t = torch.tensor([te], dtype=torch.float64, device=dev)
-        if dist: dist.all_reduce(te_t, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * wl.pairs * ksteps / float(te_t.item()) / 1e9, "unit": UNIT,
+        te_max = max_over_ranks(te, dist, dev)
+        e2e = {"value": whole_job_rate(wl.pairs, ksteps, world, te_max), "unit": UNIT,
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "steps": ksteps,
-               "ms_per_step": float(te_t.item()) / ksteps * 1e3, "api": "nb_regular_force_host (pinned host buffers)"}
+               "ms_per_step": te_max / ksteps * 1e3, "api": "nb_regular_force_host (pinned host buffers)"}
         ctx.nb_set_j(*state_dev)
 
     if rank != 0:
@@ -253,11 +271,16 @@ def run_gpu_arm(args):
         "config": workload_config(wl, args.config),
         "fp32_peak_fraction": value / world * 1e9 * FLOPS_PER_PAIR / (peak_tf * 1e12),
         "roofline": {"bound": "alu", "kernel": "force_kernel", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                     "frac": ach_tf / peak_tf, "traffic": None,
-                     "note": f"achieved = N_i*N pairs x {FLOPS_PER_PAIR:.0f} flop / force-kernel time (CUDA events, "
-                             f"includes the gather kernel when the j-range is split); peak = {nsm} SMs x 128 FP32 "
-                             f"lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz, "
-                             f"{peaks['src']})", "ms": t_force * 1e3},
+                     "frac": ach_tf / peak_tf,
+                     "traffic": FORCE_DRAM_BYTES_C5 if (args.config == 5 and args.n_i is None) else None,
+                     "fma_pipe_busy": wl.pairs * LANE_SLOTS_PER_PAIR / t_force / (nsm * 128 * peaks["sm_max_mhz"] * 1e6),
+                     "note": f"achieved = N_i*N pairs x {FLOPS_PER_PAIR:.0f} flop (convention) / time of "
+                             f"nb_regular_force on its stream (CUDA events; force_kernel plus the small "
+                             f"reduce_gather_kernel of the j-split rows); peak = {nsm} SMs x 128 FP32 lanes x 2 x "
+                             f"{peaks['sm_max_mhz']:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz, {peaks['src']}; the "
+                             f"file holds no FP32 figure, DESIGN.md section 7 derives this one); fma_pipe_busy = "
+                             f"{LANE_SLOTS_PER_PAIR:.0f} issued FP32 lane-slots per pair / 128 per clock per SM",
+                     "ms": t_force * 1e3},
         "roofline_predictor": {"bound": "hbm", "kernel": "predict_kernel", "achieved": pred_bytes / t_pred / 1e9,
                                "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": pred_bytes / t_pred / 1e9 / peaks["hbm_gbs"],
                                "traffic": None, "ms": t_pred * 1e3,

@@ -44,9 +44,9 @@ int nb_version(void);
 const char* nb_strerror(int code);
 
 /* Bytes of device workspace nb_create needs for up to n_max j-particles, active blocks of up to n_i_max rows
- * and neighbour lists of nbr_cap entries per row.  Holds the packed predicted j-records (40 B per j) and, for
- * the j-split path (small active blocks), per-(row, j-chunk) partial sums, counts and lists.
- * Returns 0 if an argument is invalid. */
+ * and neighbour lists of nbr_cap entries per row (1 <= nbr_cap <= 8192).  Holds the packed predicted j-records
+ * (40 B per j) and, for the row blocks whose j-range is split over several CTAs, 48 B of
+ * partial sums per (row, j-chunk): at most 96 MB.  Returns 0 if an argument is invalid. */
 size_t nb_workspace_bytes(int64_t n_max, int64_t n_i_max, int32_t nbr_cap);
 
 /* cf. GPUNB_OPEN(NTOT).  Creates a context on CUDA device `device`.
@@ -91,7 +91,9 @@ int nb_get_predicted(nb_ctx* ctx, double* xp, double* vp, void* stream);
  *   acc, jerk:  dev double[n_i][3]
  *   nbr_count:  dev int32[n_i]   TRUE number of neighbours (may exceed nbr_cap: overflow, not an error)
  *   nbr_list:   dev int32[n_i][nbr_cap]  row q valid in [0, min(count, nbr_cap)), ascending j; the self index
- *               is never listed or counted; entries past the count are left untouched
+ *               is never listed or counted; entries past the count are left untouched.  An overflowed row
+ *               (count > nbr_cap) holds nbr_cap of its neighbours: the first ones in j if the row ran in one
+ *               CTA, otherwise whichever reserved a slot first (reading R7/R15 in DESIGN.md)
  *   n_overflow: dev int32[1]     number of rows with count > nbr_cap
  * The pair within 1e-6 (relative) of r_s may fall on either side of the test (fp32 squares). */
 int nb_regular_force(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const double* r_s, double t, double* acc,
