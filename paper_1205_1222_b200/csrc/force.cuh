@@ -27,6 +27,14 @@
 
 namespace nbreg {
 
+// Far/near split: pairs farther than kappa X (X = largest |coordinate| of i) may skip the low words; kappa = 1/4.
+// A smaller kappa makes the near path rarer (kappa = 1/8: +5 % throughput at N = 2^20) but doubles the far path's
+// per-pair position error, and the worst jerk rows of config 5 then pass 1e-5 (measured).
+#ifndef NBREG_KAPPA2
+#define NBREG_KAPPA2 0.0625f
+#endif
+constexpr float kFarFraction2 = NBREG_KAPPA2;
+
 struct ForceArgs {
     const float4* packed;   // packed j-pair records, n_pad / 2 pairs
     int32_t n;              // real j-particles
@@ -256,7 +264,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         I[u].h2 = live ? fmaxf(h2, 1.17549435e-38f) : -1.f;
         // far threshold: beyond r_s with a 2^-10 margin, and beyond X/4 (X = largest |coordinate| of i), see above
         const float xmax = fmaxf(fabsf(xh), fmaxf(fabsf(yh), fabsf(zh)));
-        I[u].hfar2 = live ? fmaxf(I[u].h2 * 1.0009765625f, 0.0625f * xmax * xmax) : -1.f;
+        I[u].hfar2 = live ? fmaxf(I[u].h2 * 1.0009765625f, kFarFraction2 * xmax * xmax) : -1.f;
         I[u].self = i;
         I[u].nlim = (live && h2 >= 1.17549435e-38f) ? a.n : 0;
         I[u].cnt = 0;

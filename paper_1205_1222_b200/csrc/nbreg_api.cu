@@ -215,10 +215,17 @@ Plan make_plan(const Machine* c, int32_t n_i, int64_t opt_i_block, int64_t opt_j
     return best;
 }
 
+// two j-tile stages + their mbarriers
+size_t force_smem_bytes(int ipt, int warps, int jt) {
+    (void)ipt;
+    (void)warps;
+    return 2 * (size_t)jt * kBytesPerJ + 2 * sizeof(uint64_t);
+}
+
 template <int IPT, int WARPS, int JT, int MINB>
 int query_force(int* per_sm) {
     auto kern = force_kernel<IPT, WARPS, JT, MINB>;
-    const size_t smem = 2 * (size_t)JT * kBytesPerJ + 2 * sizeof(uint64_t);
+    const size_t smem = force_smem_bytes(IPT, WARPS, JT);
     NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     NB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, WARPS * 32, smem));
     return NB_OK;
@@ -226,7 +233,7 @@ int query_force(int* per_sm) {
 
 template <int IPT, int WARPS, int JT, int MINB>
 int launch_force(const Plan& p, const ForceArgs& fa, cudaStream_t st) {
-    const size_t smem = 2 * (size_t)JT * kBytesPerJ + 2 * sizeof(uint64_t);
+    const size_t smem = force_smem_bytes(IPT, WARPS, JT);
     force_kernel<IPT, WARPS, JT, MINB><<<p.grid, WARPS * 32, smem, st>>>(fa);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
