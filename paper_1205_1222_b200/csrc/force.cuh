@@ -54,9 +54,12 @@ struct ForceArgs {
     double* jerk;
     int32_t* nbr_count;
     int32_t* nbr_list;
-    int32_t* n_overflow;
+    int32_t* n_overflow;    // not touched here: reduce_gather_kernel publishes it
+    // zero-between-calls scratch in the workspace (reduce_gather_kernel leaves it zeroed again):
+    int32_t* slot_count;    // [tail rows] list-slot counters of the j-split rows
+    int32_t* overflow_ws;   // [1] rows with count > cap found so far in this call
     // partial sums of the tail blocks, indexed by tail row = row - main_blocks * rows_per_cta: [tail row][S][6].
-    // Their list entries go straight to nbr_list through an atomic slot counter in nbr_count (zeroed by the host).
+    // Their list entries go straight to nbr_list through the atomic slot counters slot_count.
     double* part_sum;
 };
 
@@ -307,7 +310,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
                     geom_lo(xl, q4, I[u], g[u]);
                     const bool nb0 = g[u].r2.x < I[u].h2;  // eq. (2)/(11): neighbour iff r^2 < r_s^2
                     const bool nb1 = g[u].r2.y < I[u].h2;
-                    int32_t* shared_count = split ? a.nbr_count + rows[u] : nullptr;
+                    int32_t* shared_count = split ? a.slot_count + (rows[u] - tail_row0) : nullptr;
                     append(I[u], j, nb0, a.cap, shared_count);
                     append(I[u], j + 1, nb1, a.cap, shared_count);
                     if (nb0) g[u].r2.x = __int_as_float(0x7f800000);
@@ -343,7 +346,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
                 a.jerk[row * 3 + c] = sum[u][3 + c];
             }
             a.nbr_count[row] = I[u].cnt;
-            if (I[u].cnt > a.cap) atomicAdd(a.n_overflow, 1);
+            if (I[u].cnt > a.cap) atomicAdd(a.overflow_ws, 1);
         } else {
             flush_pending(I[u], a.cap);
             const size_t pi = (size_t)(row - tail_row0) * a.n_chunks + chunk;

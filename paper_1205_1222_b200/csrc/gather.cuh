@@ -2,7 +2,8 @@
 //
 // "partial forces and partial neighbour lists ... are distributed for multiple thread-blocks ... we prepared
 // kernels for force reduction and list gathering ... Partial forces are summed and sparsely scattered partial
-// lists are serialized to a linear array".  Here: one warp per j-split row.
+// lists are serialized to a linear array".  Here: one warp per j-split row.  The kernel runs
+// after every force launch (with no rows if nothing was split): its last block publishes n_overflow.
 //   Sums: fp64; lanes stride over the row's j-chunks, then a fixed xor-shuffle tree: deterministic.
 //   Lists: the chunks' CTAs appended their neighbours to the row's final list in arrival order (atomic slot
 //   counter, force.cuh).  Each chunk covers a contiguous j-range and its entries arrive in ascending j, so the
@@ -24,9 +25,13 @@ struct GatherArgs {
     const double* part_sum;    // [split rows][S][6]
     double* acc;
     double* jerk;
-    const int32_t* nbr_count;  // final (true) counts, complete when this kernel starts
+    int32_t* nbr_count;
     int32_t* nbr_list;
     int32_t* n_overflow;
+    // zero-between-calls scratch (see ForceArgs): this kernel consumes it and leaves it zeroed for the next call
+    int32_t* slot_count;       // [split rows] true counts of the j-split rows, complete when this kernel starts
+    int32_t* overflow_ws;      // [1]
+    int32_t* ticket;           // [1] blocks of this kernel that are done
 };
 
 constexpr int kGatherWarps = 4;
@@ -37,7 +42,7 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
     const int warp = threadIdx.x >> 5;
     const int64_t prow = (int64_t)blockIdx.x * kGatherWarps + warp;  // row among the split rows
     const int64_t row = a.row0 + prow;
-    if (row >= a.n_i) return;  // warp-uniform
+    if (row < a.n_i) {  // warp-uniform
     const int S = a.n_chunks;
     const size_t rbase = (size_t)prow * S;
 
@@ -59,7 +64,12 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
     }
 
     // ---- list: stable counting sort of the stored entries by chunk number
-    const int32_t cnt = a.nbr_count[row];  // true count, may exceed cap
+    const int32_t cnt = a.slot_count[prow];  // true count, may exceed cap
+    __syncwarp();
+    if (lane == 0) {
+        a.nbr_count[row] = cnt;
+        a.slot_count[prow] = 0;
+    }
     const int32_t stored = min(cnt, a.cap);
     int32_t* out = a.nbr_list + (size_t)row * a.cap;
     int32_t* stage = stage_all + (size_t)warp * (a.cap + S);
@@ -102,7 +112,18 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
         if (valid && before == 0) bin[c] += __popc(peers);
         __syncwarp();
     }
-    if (lane == 0 && cnt > a.cap) atomicAdd(a.n_overflow, 1);
+    if (lane == 0 && cnt > a.cap) atomicAdd(a.overflow_ws, 1);
+    }  // row < n_i
+
+    // ---- the last block to finish publishes the overflow count of the whole call and re-zeroes the scratch
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(a.ticket, 1) == (int32_t)gridDim.x - 1) {
+            *a.n_overflow = atomicExch(a.overflow_ws, 0);
+            *a.ticket = 0;
+        }
+    }
 }
 
 }  // namespace nbreg

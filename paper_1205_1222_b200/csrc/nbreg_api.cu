@@ -61,6 +61,8 @@ struct Plan {
 struct WorkspaceLayout {
     size_t packed_off, packed_bytes;
     size_t psum_off, psum_bytes;
+    size_t slot_off, slot_bytes;   // int32 list-slot counters of the j-split rows (zero between calls)
+    size_t ctl_off, ctl_bytes;     // int32 {overflow count, gather ticket} (zero between calls)
     int64_t row_chunk_limit;  // (row, j-chunk) slots of partial sums
     size_t total;
 };
@@ -84,6 +86,8 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
     };
     place((size_t)n_pad * kBytesPerJ, w.packed_off, w.packed_bytes);
     place((size_t)w.row_chunk_limit * 6 * sizeof(double), w.psum_off, w.psum_bytes);
+    place((size_t)(n_i_max + 512) * sizeof(int32_t), w.slot_off, w.slot_bytes);
+    place(64, w.ctl_off, w.ctl_bytes);
     w.total = off;
     return w;
 }
@@ -342,6 +346,14 @@ int nb_create(nb_ctx** out, int device, int64_t n_max, int64_t n_i_max, int32_t 
         }
         c->ws_owned = true;
     }
+    // the list-slot counters and the control words are zero between calls: the gather kernel re-zeroes what a
+    // call used, so they are cleared once, here
+    if (cudaMemset(c->ws + c->lay.slot_off, 0, c->lay.ctl_off + c->lay.ctl_bytes - c->lay.slot_off) != cudaSuccess) {
+        const int rc = cuda_fail(cudaGetLastError(), "cudaMemset(workspace scratch)");
+        if (c->ws_owned) cudaFree(c->ws);
+        delete c;
+        return rc;
+    }
     *out = c;
     return NB_OK;
 }
@@ -404,8 +416,8 @@ int nb_regular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const double*
         if (rc != NB_OK) return rc;
         ++launches;
     }
-    NB_CUDA(cudaMemsetAsync(n_overflow, 0, sizeof(int32_t), st));
     if (n_i == 0) {
+        NB_CUDA(cudaMemsetAsync(n_overflow, 0, sizeof(int32_t), st));
         c->info[5] = launches;
         return NB_OK;
     }
@@ -431,18 +443,21 @@ int nb_regular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const double*
     const Shape& sh = kShapes[p.shape];
     const int64_t row0 = (int64_t)p.main_blocks * sh.rows;
     const bool has_split = p.n_chunks > 1 && row0 < n_i;
-    if (has_split)  // the split rows' CTAs reserve list slots with atomics on the final counts
-        NB_CUDA(cudaMemsetAsync(nbr_count + row0, 0, (size_t)(n_i - row0) * sizeof(int32_t), st));
+    int32_t* ctl = reinterpret_cast<int32_t*>(c->ws + c->lay.ctl_off);
+    fa.slot_count = reinterpret_cast<int32_t*>(c->ws + c->lay.slot_off);
+    fa.overflow_ws = ctl;
     int rc = force_dispatch(p.shape, nullptr, &p, &fa, st);
     if (rc != NB_OK) return rc;
     ++launches;
-    if (has_split) {
+    {  // S5 + n_overflow: always launched, with no rows when nothing was split
         GatherArgs ga{};
-        ga.row0 = (int32_t)row0; ga.n_i = n_i; ga.n_chunks = p.n_chunks; ga.cap = c->cap;
+        ga.row0 = (int32_t)(has_split ? row0 : n_i); ga.n_i = n_i; ga.n_chunks = p.n_chunks; ga.cap = c->cap;
         ga.chunk_j = p.tiles_per_chunk * sh.jt;
         ga.part_sum = fa.part_sum;
         ga.acc = acc; ga.jerk = jerk; ga.nbr_count = nbr_count; ga.nbr_list = nbr_list; ga.n_overflow = n_overflow;
-        const unsigned blocks = (unsigned)((n_i - row0 + kGatherWarps - 1) / kGatherWarps);
+        ga.slot_count = fa.slot_count; ga.overflow_ws = ctl; ga.ticket = ctl + 1;
+        const int64_t split_rows = has_split ? n_i - row0 : 0;
+        const unsigned blocks = (unsigned)std::max<int64_t>(1, (split_rows + kGatherWarps - 1) / kGatherWarps);
         const size_t stage = (size_t)kGatherWarps * (c->cap + p.n_chunks) * sizeof(int32_t);
         reduce_gather_kernel<<<blocks, kGatherWarps * 32, stage, st>>>(ga);
         NB_CUDA(cudaGetLastError());
