@@ -16,6 +16,12 @@
  *   oracle_force_given_lists same sums, "neighbour" := membership in a given list (for rows whose GPU list
  *                            differs from the oracle's only by pairs inside the 1e-6 boundary band, north_star).
  *
+ *   oracle_regular_force_ex  the two variants the paper's own kernel has (Listing B2): the
+ *                            velocity neighbour criterion eq. (3), PAPER.md:69-73,
+ *                            R_min = min(|R_ij|, |R_ij + dtr_i V_ij|) < h_i (lines 17-19, 22, 26 of the listing), and
+ *                            the potential sum "fo.pot += mrinv1": pot_i = sum m_j / r_ij over
+ *                            the same non-neighbours as eq. (9) (sign as in the listing: positive).
+ *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC oracle.c -o liboracle.so -lm
  * (-ffp-contract=off: no FMA contraction, so the arithmetic is exactly what is written.)
  */
@@ -146,5 +152,51 @@ void oracle_force_given_lists(int64_t n, const double* xp, const double* vp, con
             jerk[3 * q + c] = jk[c];
         }
         free(sorted);
+    }
+}
+
+/* Eq. (9), (10), (11) with the VELOCITY criterion eq. (3) and the potential of Listing B2.
+ *   dtr [n_i] (may be NULL = all zero): the regular time-step of row q; neighbour iff
+ *       min(|R|^2, |R + dtr V|^2) < r_s^2      (Listing B2: "if (fminf(r2, r2p) < ip.h2)"),
+ *   compared on squares, strictly.  dtr = 0 gives oracle_regular_force exactly.
+ *   pot [n_i] (may be NULL): sum over the summed (non-neighbour) pairs of m_j / r   ("fo.pot += mrinv1").
+ * Everything else as oracle_regular_force (self by index, coincident pairs, true count, ascending list). */
+void oracle_regular_force_ex(int64_t n, const double* xp, const double* vp, const double* m, int64_t n_i,
+                             const int32_t* i_idx, const double* r_s, const double* dtr, double* acc, double* jerk,
+                             double* pot, int32_t* count, int32_t* list, int64_t list_stride) {
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t q = 0; q < n_i; ++q) {
+        int64_t i = i_idx[q];
+        double h2 = r_s[q] * r_s[q];
+        double dt = dtr ? dtr[q] : 0.0;
+        double a[3] = {0.0, 0.0, 0.0}, jk[3] = {0.0, 0.0, 0.0}, phi = 0.0;
+        int32_t cnt = 0;
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            double R[3], V[3], Rp[3];
+            for (int c = 0; c < 3; ++c) {
+                R[c] = xp[3 * j + c] - xp[3 * i + c];
+                V[c] = vp[3 * j + c] - vp[3 * i + c];
+                Rp[c] = R[c] + dt * V[c];
+            }
+            double r2 = R[0] * R[0] + R[1] * R[1] + R[2] * R[2];
+            double r2p = Rp[0] * Rp[0] + Rp[1] * Rp[1] + Rp[2] * Rp[2];
+            double rmin2 = r2p < r2 ? r2p : r2;
+            if (rmin2 < h2) {
+                if (list && cnt < list_stride) list[q * list_stride + cnt] = (int32_t)j;
+                ++cnt;
+            } else if (r2 == 0.0) {
+                continue;
+            } else {
+                pair_term(R, V, r2, m[j], a, jk);
+                phi += m[j] / sqrt(r2);
+            }
+        }
+        for (int c = 0; c < 3; ++c) {
+            acc[3 * q + c] = a[c];
+            jerk[3 * q + c] = jk[c];
+        }
+        if (pot) pot[q] = phi;
+        count[q] = cnt;
     }
 }

@@ -39,6 +39,8 @@ def _load():
                                              _f64p, _f64p, _i32p, _i32p, ctypes.c_int64]
         lib.oracle_force_given_lists.argtypes = [ctypes.c_int64, _f64p, _f64p, _f64p, ctypes.c_int64, _i32p, _i32p,
                                                  _i32p, ctypes.c_int64, _f64p, _f64p]
+        lib.oracle_regular_force_ex.argtypes = [ctypes.c_int64, _f64p, _f64p, _f64p, ctypes.c_int64, _i32p, _f64p,
+                                                _f64p, _f64p, _f64p, _f64p, _i32p, _i32p, ctypes.c_int64]
         _lib = lib
     return _lib
 
@@ -102,6 +104,32 @@ def regular_force(xp, vp, m, i_idx, r_s, list_stride: int = 256, want_lists: boo
             break
         stride = mx
     return acc, jerk, count, [lists[q, : count[q]].copy() for q in range(n_i)]
+
+
+def regular_force_ex(xp, vp, m, i_idx, r_s, dtr=None, list_stride: int = 256):
+    """Variants of Listing B2: velocity criterion eq. (3) with per-row regular step dtr
+    (None = plain criterion) and the potential sum.  Returns acc, jerk, pot, count, lists."""
+    xp, vp, m, r_s = map(_d, (xp, vp, m, r_s))
+    i_idx = np.ascontiguousarray(i_idx, dtype=np.int32)
+    n, n_i = xp.shape[0], i_idx.shape[0]
+    dtr_p = None
+    if dtr is not None:
+        dtr = _d(dtr)
+        dtr_p = _p(dtr)
+    acc = np.empty((n_i, 3))
+    jerk = np.empty((n_i, 3))
+    pot = np.empty(n_i)
+    count = np.empty(n_i, dtype=np.int32)
+    stride = max(1, int(list_stride))
+    while True:
+        lists = np.empty((n_i, stride), dtype=np.int32)
+        _load().oracle_regular_force_ex(n, _p(xp), _p(vp), _p(m), n_i, _pi(i_idx), _p(r_s), dtr_p, _p(acc), _p(jerk),
+                                        _p(pot), _pi(count), _pi(lists), stride)
+        mx = int(count.max()) if n_i else 0
+        if mx <= stride:
+            break
+        stride = mx
+    return acc, jerk, pot, count, [lists[q, : count[q]].copy() for q in range(n_i)]
 
 
 def force_given_lists(xp, vp, m, i_idx, lists, counts=None):

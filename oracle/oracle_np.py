@@ -39,3 +39,33 @@ def regular_force(xp, vp, m, i_idx, r_s):
         lists.append(np.nonzero(nb)[0].astype(np.int32))
     count = np.array([len(l) for l in lists], dtype=np.int32)
     return acc, jerk, count, lists
+
+
+def regular_force_ex(xp, vp, m, i_idx, r_s, dtr=None):
+    """Velocity criterion eq. (3) and the potential of Listing B2, written
+    from the equations: neighbour iff min(|R|, |R + dtr V|) < r_s; pot = sum m / r over the summed pairs."""
+    xp = np.asarray(xp, dtype=np.float64)
+    vp = np.asarray(vp, dtype=np.float64)
+    m = np.asarray(m, dtype=np.float64)
+    n_i = len(i_idx)
+    dtr = np.zeros(n_i) if dtr is None else np.asarray(dtr, dtype=np.float64)
+    acc = np.zeros((n_i, 3))
+    jerk = np.zeros((n_i, 3))
+    pot = np.zeros(n_i)
+    lists = []
+    for q, (i, h) in enumerate(zip(i_idx, r_s)):
+        R = xp - xp[i]
+        V = vp - vp[i]
+        r = np.linalg.norm(R, axis=1)
+        rp = np.linalg.norm(R + dtr[q] * V, axis=1)
+        other = np.arange(xp.shape[0]) != i
+        nb = other & (np.minimum(r * r, rp * rp) < h * h)
+        summed = other & ~nb & (r > 0.0)
+        Rs, Vs, rs_, ms = R[summed], V[summed], r[summed], m[summed]
+        rv = np.einsum("jc,jc->j", Rs, Vs)
+        acc[q] = (ms[:, None] * Rs / rs_[:, None] ** 3).sum(axis=0)
+        jerk[q] = (ms[:, None] * (Vs / rs_[:, None] ** 3 - 3.0 * rv[:, None] * Rs / rs_[:, None] ** 5)).sum(axis=0)
+        pot[q] = (ms / rs_).sum()
+        lists.append(np.nonzero(nb)[0].astype(np.int32))
+    count = np.array([len(l) for l in lists], dtype=np.int32)
+    return acc, jerk, pot, count, lists

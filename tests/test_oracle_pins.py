@@ -248,3 +248,120 @@ def test_thread_count_does_not_change_results():
     a1, j1, c1, _ = oracle.regular_force(x, v, m, idx, rs)
     oracle.set_num_threads(nt)
     assert np.array_equal(a, a1) and np.array_equal(j, j1) and np.array_equal(c, c1)
+
+
+# ================================================================ NEXT-1: velocity criterion eq. (3) and potential
+@pytest.mark.parametrize("impl", [oracle, oracle_np])
+def test_p11_velocity_criterion_two_body(impl):
+    g = GOLD["P11_velocity_criterion_two_body"]
+    xp = np.array([g["xi"], g["xj"]], dtype=float)
+    vp = np.array([g["vi"], g["vj"]], dtype=float)
+    m = np.array([7.0, g["mj"]])
+    ii = np.array([0], dtype=np.int32)
+    for case in g["cases"]:
+        acc, jerk, pot, cnt, lists = impl.regular_force_ex(xp, vp, m, ii, np.array([case["r_s"]]),
+                                                           np.array([case["dtr"]]))
+        if case["neighbour"]:
+            assert cnt[0] == 1 and list(lists[0]) == [1], case
+            assert np.all(acc == 0) and np.all(jerk == 0) and pot[0] == 0
+        else:
+            assert cnt[0] == 0, case
+            np.testing.assert_allclose(acc[0], g["acc"], rtol=0, atol=1e-17)
+            np.testing.assert_allclose(jerk[0], g["jerk"], rtol=0, atol=1e-17)
+            np.testing.assert_allclose(pot[0], g["pot"], rtol=0, atol=1e-16)
+
+
+@pytest.mark.parametrize("impl", [oracle, oracle_np])
+def test_p12_potential_ring(impl):
+    g, gp = GOLD["P2_ring"], GOLD["P12_potential_ring"]
+    nr = g["n_ring"]
+    ang = 2 * np.pi * np.arange(nr) / nr
+    xp = np.zeros((nr + 1, 3))
+    xp[:nr, 0] = g["radius"] * np.cos(ang)
+    xp[:nr, 1] = g["radius"] * np.sin(ang)
+    xp[nr] = [0, 0, g["zi"]]
+    vp = np.zeros((nr + 1, 3))
+    m = np.full(nr + 1, g["m_each"])
+    ii = np.array([nr], dtype=np.int32)
+    _, _, pot, cnt, _ = impl.regular_force_ex(xp, vp, m, ii, np.array([g["rs_inside"]]))
+    assert cnt[0] == 0 and abs(pot[0] - gp["pot"]) < 1e-15
+    _, _, pot, cnt, _ = impl.regular_force_ex(xp, vp, m, ii, np.array([g["rs_outside"]]))
+    assert cnt[0] == nr and pot[0] == 0.0
+
+
+def test_ex_with_zero_dtr_is_the_plain_path():
+    x, v, m = _plummer(400)
+    ii = np.arange(0, 400, 3, dtype=np.int32)
+    rs = inputs.kth_neighbour_distance(x, ii, 12, brute=True) * 1.0001
+    a0, j0, c0, l0 = oracle.regular_force(x, v, m, ii, rs)
+    for dtr in (None, np.zeros(len(ii))):
+        a1, j1, _, c1, l1 = oracle.regular_force_ex(x, v, m, ii, rs, dtr)
+        assert np.array_equal(a0, a1) and np.array_equal(j0, j1) and np.array_equal(c0, c1)
+        assert all(np.array_equal(p, q) for p, q in zip(l0, l1))
+
+
+def test_velocity_lists_bruteforce_and_monotone():
+    """eq. (3) by brute force in numpy; the velocity list contains the plain list (min(...) <= |R|)."""
+    x, v, m = _plummer(96)
+    ii = np.arange(96, dtype=np.int32)
+    rs = inputs.kth_neighbour_distance(x, ii, 6, brute=True) * 1.0001
+    dtr = 2.0 ** -np.arange(96).astype(float).clip(0, 6) * 0.5
+    _, _, _, cnt, lists = oracle.regular_force_ex(x, v, m, ii, rs, dtr)
+    _, _, _, l_plain = oracle.regular_force(x, v, m, ii, rs)
+    grew = 0
+    for q in range(96):
+        R = x - x[q]
+        Rp = R + dtr[q] * (v - v[q])
+        rmin = np.minimum(np.linalg.norm(R, axis=1), np.linalg.norm(Rp, axis=1))
+        want = [j for j in range(96) if j != q and rmin[j] < rs[q]]
+        assert list(lists[q]) == want and cnt[q] == len(want)
+        assert set(l_plain[q]) <= set(want)
+        grew += len(want) > len(l_plain[q])
+    assert grew > 0  # the criterion does add fast approachers on this sample
+
+
+def test_potential_complementarity_and_energy():
+    """pot_reg + sum over the list of m/r = total potential for any r_s and dtr; sum m_i pot_i = -2 W, checked
+    against a direct double loop, and W ~ -1/2 for a Plummer model in N-body units (E = -1/4)."""
+    rngs = inputs.streams(6, 5)
+    x, v = inputs.plummer_points(rngs, 700)
+    m = np.full(700, 1.0 / 700)
+    ii = np.arange(700, dtype=np.int32)
+    rs = inputs.kth_neighbour_distance(x, ii, 10, brute=True) * 1.0001
+    _, _, pot0, _, _ = oracle.regular_force_ex(x, v, m, ii, np.zeros(700))
+    _, _, pot, cnt, lists = oracle.regular_force_ex(x, v, m, ii, rs, np.full(700, 0.05))
+    back = np.array([sum(m[j] / np.linalg.norm(x[j] - x[q]) for j in lists[q]) for q in range(700)])
+    np.testing.assert_allclose(pot + back, pot0, rtol=1e-13)
+    d = np.linalg.norm(x[:, None, :] - x[None, :, :], axis=2)
+    np.fill_diagonal(d, np.inf)
+    W = -0.5 * (m[:, None] * m[None, :] / d).sum()
+    assert abs((m * pot0).sum() + 2 * W) < 1e-13
+    assert abs(W + 0.5) < 0.05
+
+
+def test_acc_is_gradient_of_potential():
+    """d(pot_i)/d(x_i) = acc_i with the neighbour mask frozen (pot = sum m/|x_j - x_i|): central differences."""
+    x, v, m = _plummer(300)
+    ii = np.array([5, 77, 210], dtype=np.int32)
+    acc, _, _, _, _ = oracle.regular_force_ex(x, v, m, ii, np.zeros(3))
+    eps = 1e-6
+    for q, i in enumerate(ii):
+        for c in range(3):
+            xp_, xm_ = x.copy(), x.copy()
+            xp_[i, c] += eps
+            xm_[i, c] -= eps
+            pp = oracle.regular_force_ex(xp_, v, m, ii[q:q + 1], np.zeros(1))[2][0]
+            pm = oracle.regular_force_ex(xm_, v, m, ii[q:q + 1], np.zeros(1))[2][0]
+            # moving i by +eps changes R_ij by -eps: d pot / d x_i = + sum m R / r^3 = acc
+            assert abs((pp - pm) / (2 * eps) - acc[q, c]) < 2e-7 * np.linalg.norm(acc[q])
+
+
+def test_ex_c_vs_numpy():
+    x, v, m = _plummer(500)
+    ii = np.arange(0, 500, 2, dtype=np.int32)
+    rs = inputs.kth_neighbour_distance(x, ii, 14, brute=True) * 1.0001
+    dtr = np.full(len(ii), 1.0 / 32)
+    a, j, p, c, l = oracle.regular_force_ex(x, v, m, ii, rs, dtr)
+    a2, j2, p2, c2, l2 = oracle_np.regular_force_ex(x, v, m, ii, rs, dtr)
+    assert _rel(a, a2).max() < 1e-13 and _rel(j, j2).max() < 1e-12 and np.abs(p / p2 - 1).max() < 1e-13
+    assert np.array_equal(c, c2) and all(np.array_equal(p_, q_) for p_, q_ in zip(l, l2))
