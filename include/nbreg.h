@@ -45,8 +45,8 @@ const char* nb_strerror(int code);
 
 /* Bytes of device workspace nb_create needs for up to n_max j-particles, active blocks of up to n_i_max rows
  * and neighbour lists of nbr_cap entries per row (1 <= nbr_cap <= 8192).  Holds the packed predicted j-records
- * (40 B per j) and, for the row blocks whose j-range is split over several CTAs, 48 B of
- * partial sums per (row, j-chunk): at most 96 MB, plus 4 B per row of list-slot counters.  nb_create clears the
+ * (40 B per j) and, for the row blocks whose j-range is split over several CTAs, 56 B of
+ * partial sums per (row, j-chunk): at most 112 MB, plus 4 B per row of list-slot counters.  nb_create clears the
  * counters once; every call leaves them cleared.  Returns 0 if an argument is invalid. */
 size_t nb_workspace_bytes(int64_t n_max, int64_t n_i_max, int32_t nbr_cap);
 
@@ -99,6 +99,18 @@ int nb_get_predicted(nb_ctx* ctx, double* xp, double* vp, void* stream);
  * The pair within 1e-6 (relative) of r_s may fall on either side of the test (fp32 squares). */
 int nb_regular_force(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const double* r_s, double t, double* acc,
                      double* jerk, int32_t* nbr_count, int32_t* nbr_list, int32_t* n_overflow, void* stream);
+
+/* The two variants of the paper's own kernel (Listing B2), selected by non-NULL pointers:
+ *   dtr: dev double[n_i] or NULL.  Regular time-step of each row for the VELOCITY neighbour criterion eq. (3),
+ *        j is a neighbour iff min(|R_ij|^2, |R_ij + dtr V_ij|^2) < r_s^2 ("fminf(r2, r2p) < ip.h2",
+ *        PAPER.md:381); everything else (what is summed, what is listed) follows from that as in
+ *        nb_regular_force.  dtr = 0 reproduces nb_regular_force exactly; NULL selects the plain-criterion kernel.
+ *   pot: dev double[n_i] or NULL.  pot[q] = sum of m_j / r_ij over the summed (non-neighbour) pairs
+ *        ("fo.pot += mrinv1"; positive, as in the listing).
+ * All other arguments, conventions and return codes as nb_regular_force. */
+int nb_regular_force_ex(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const double* r_s, const double* dtr,
+                        double t, double* acc, double* jerk, double* pot, int32_t* nbr_count, int32_t* nbr_list,
+                        int32_t* n_overflow, void* stream);
 
 /* End-to-end convenience with HOST buffers: copies the j-state and the active block to device buffers the
  * context owns (allocated on first use, sized by n_max / n_i_max / nbr_cap), runs nb_set_j + nb_regular_force

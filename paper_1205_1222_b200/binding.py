@@ -48,6 +48,7 @@ def load(build_if_missing: bool = True):
     lib.nb_predict_j.argtypes = [vp, dbl, vp]
     lib.nb_get_predicted.argtypes = [vp, vp, vp, vp]
     lib.nb_regular_force.argtypes = [vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp, vp]
+    lib.nb_regular_force_ex.argtypes = [vp, i32, vp, vp, vp, dbl, vp, vp, vp, vp, vp, vp, vp]
     lib.nb_regular_force_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp]
     lib.nb_set_option.argtypes = [vp, ctypes.c_char_p, i64]
     lib.nb_last_launch_info.argtypes = [vp, ctypes.POINTER(i64)]
@@ -159,6 +160,23 @@ class Context:
         _check(self.lib.nb_regular_force(
             self._h, n_i, _dev(i_idx, torch.int32, "i_idx"), _dev(r_s, torch.float64, "r_s"), float(t),
             _dev(out["acc"], torch.float64, "acc"), _dev(out["jerk"], torch.float64, "jerk"),
+            _dev(out["nbr_count"], torch.int32, "nbr_count"), _dev(out["nbr_list"], torch.int32, "nbr_list"),
+            _dev(out["n_overflow"], torch.int32, "n_overflow"), _stream_ptr(stream)))
+        return out
+
+    # -- nb_regular_force_ex: velocity criterion (dtr) and / or potential output (out["pot"])
+    def nb_regular_force_ex(self, i_idx, r_s, t: float, dtr=None, want_pot: bool = False, out=None, stream=None):
+        n_i = int(i_idx.shape[0])
+        if out is None:
+            out = self.alloc_outputs(n_i)
+        if want_pot and "pot" not in out:
+            out["pot"] = torch.empty(n_i, dtype=torch.float64, device=self.workspace.device)
+        null = ctypes.c_void_p()
+        _check(self.lib.nb_regular_force_ex(
+            self._h, n_i, _dev(i_idx, torch.int32, "i_idx"), _dev(r_s, torch.float64, "r_s"),
+            null if dtr is None else _dev(dtr, torch.float64, "dtr"), float(t),
+            _dev(out["acc"], torch.float64, "acc"), _dev(out["jerk"], torch.float64, "jerk"),
+            _dev(out["pot"], torch.float64, "pot") if want_pot else null,
             _dev(out["nbr_count"], torch.int32, "nbr_count"), _dev(out["nbr_list"], torch.int32, "nbr_list"),
             _dev(out["n_overflow"], torch.int32, "n_overflow"), _stream_ptr(stream)))
         return out

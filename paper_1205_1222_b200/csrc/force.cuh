@@ -49,6 +49,9 @@ struct ForceArgs {
     int32_t cap;
     const int32_t* i_idx;
     const double* r_s;
+    const double* dtr;       // VEL: regular time-step per row, eq. (3)
+    const float* tile_vmax;  // VEL: speed bound per 256 consecutive j (predict.cuh)
+    double* pot;             // POT: sum m_j / r over the summed pairs ("fo.pot += mrinv1")
     // final outputs (main blocks)
     double* acc;
     double* jerk;
@@ -118,6 +121,11 @@ struct IState {
     float nxh, nyh, nzh, nxl, nyl, nzl, nvx, nvy, nvz;
     float h2;        // r_s^2 in fp32, clamped to >= FLT_MIN so that the self pair (r^2 = 0) is always masked
     float hfar2;     // pairs with |R_hi|^2 >= hfar2 take the far path (no low words, surely not a neighbour)
+    // velocity criterion only: hfar2 is refreshed per j-tile as max(hfar_x, hfar_r + dtr vmax_tile)^2, so that a far
+    // pair cannot come within r_s during dtr either: |R + dtr V| >= |R| - dtr (|v_i| + |v_j|)
+    float hfar_x;    // kappa X
+    float hfar_r;    // r_s (1 + 2^-11) + dtr |v_i|
+    float dtr;
     int32_t self;    // own j-index (never listed)
     int32_t nlim;    // list entries must have j < nlim: n for a normal row, 0 when r_s = 0 (reading R4/R5)
     int32_t cnt;     // main path: neighbours found so far
@@ -127,10 +135,11 @@ struct IState {
 
 struct Accum {
     float2 ax, ay, az, jx, jy, jz;  // fp32 partial sums of the current j-tile; .x from j0, .y from j1
+    float2 pot;                     // used by the POT variant only
 };
 
 __device__ __forceinline__ void accum_zero(Accum& s) {
-    s.ax = s.ay = s.az = s.jx = s.jy = s.jz = make_float2(0.f, 0.f);
+    s.ax = s.ay = s.az = s.jx = s.jy = s.jz = s.pot = make_float2(0.f, 0.f);
 }
 
 __device__ __forceinline__ float2 bc(float a) { return make_float2(a, a); }
@@ -166,6 +175,8 @@ __device__ __forceinline__ void geom_lo(const float2& xl, const float4& q4, cons
 }
 
 // eq. (9), (10) for the two pairs: 3 FADD2 (V), 3 (R.V), 2 (m/r^3), 2 (alpha), 9 FFMA2 (sums); 2 MUFU.RSQ + 2 MUFU.RCP.
+// POT adds one packed add: pot += m ri (Listing B2: "fo.pot += mrinv1").
+template <bool POT>
 __device__ __forceinline__ void pair_sum(const float4& q1, const float4& q2, const float2& vz, const IState& I,
                                          const PairGeom& g, Accum& s) {
     const float2 dvx = __fadd2_rn(make_float2(q2.x, q2.y), bc(I.nvx));
@@ -174,7 +185,9 @@ __device__ __forceinline__ void pair_sum(const float4& q1, const float4& q2, con
     const float2 rv = __ffma2_rn(g.dz, dvz, __ffma2_rn(g.dy, dvy, __fmul2_rn(g.dx, dvx)));
     const float2 ri = make_float2(rsqrt_approx(g.r2.x), rsqrt_approx(g.r2.y));
     const float2 ri2 = make_float2(rcp_approx(g.r2.x), rcp_approx(g.r2.y));
-    const float2 mri3 = __fmul2_rn(__fmul2_rn(make_float2(q1.z, q1.w), ri), ri2);
+    const float2 mri = __fmul2_rn(make_float2(q1.z, q1.w), ri);
+    const float2 mri3 = __fmul2_rn(mri, ri2);
+    if (POT) s.pot = __fadd2_rn(s.pot, mri);
     const float2 al = __fmul2_rn(__fmul2_rn(rv, ri2), bc(-3.f));
     s.ax = __ffma2_rn(mri3, g.dx, s.ax);
     s.ay = __ffma2_rn(mri3, g.dy, s.ay);
@@ -182,6 +195,19 @@ __device__ __forceinline__ void pair_sum(const float4& q1, const float4& q2, con
     s.jx = __ffma2_rn(mri3, __ffma2_rn(al, g.dx, dvx), s.jx);
     s.jy = __ffma2_rn(mri3, __ffma2_rn(al, g.dy, dvy), s.jy);
     s.jz = __ffma2_rn(mri3, __ffma2_rn(al, g.dz, dvz), s.jz);
+}
+
+// Velocity criterion eq. (3), near path only: r_min^2 = min(|R|^2, |R + dtr V|^2) with the full-precision R
+// (Listing B2 lines 17-19, 22, 26).
+__device__ __forceinline__ float2 rmin2_velocity(const float4& q2, const float2& vz, const IState& I, const PairGeom& g) {
+    const float2 dvx = __fadd2_rn(make_float2(q2.x, q2.y), bc(I.nvx));
+    const float2 dvy = __fadd2_rn(make_float2(q2.z, q2.w), bc(I.nvy));
+    const float2 dvz = __fadd2_rn(vz, bc(I.nvz));
+    const float2 px = __ffma2_rn(bc(I.dtr), dvx, g.dx);
+    const float2 py = __ffma2_rn(bc(I.dtr), dvy, g.dy);
+    const float2 pz = __ffma2_rn(bc(I.dtr), dvz, g.dz);
+    const float2 r2p = __ffma2_rn(pz, pz, __ffma2_rn(py, py, __fmul2_rn(px, px)));
+    return make_float2(fminf(g.r2.x, r2p.x), fminf(g.r2.y, r2p.y));
 }
 
 // S4: "the index j is written to the neighbour list in the memory".  A main-path row is owned by
@@ -207,8 +233,9 @@ __device__ __forceinline__ void append(IState& I, int32_t j, bool nb, int32_t ca
     }
 }
 
-template <int IPT, int WARPS, int JT, int MINB>
+template <int IPT, int WARPS, int JT, int MINB, bool VEL, bool POT>
 __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
+    constexpr int kSums = POT ? 7 : 6;  // fp64 running sums per row: acc, jerk (, pot)
     constexpr int kThreads = WARPS * 32;
     constexpr int kRows = kThreads * IPT;
     constexpr int kTileQuads = JT / 2 * kQuadsPerPair;
@@ -245,7 +272,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
     // ---- S2: i-setup.  Gather the active particles' predicted state from the packed records by index.
     IState I[IPT];
     Accum s[IPT];
-    double sum[IPT][6];
+    double sum[IPT][kSums];
     int64_t rows[IPT];
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
@@ -268,6 +295,13 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         // far threshold: beyond r_s with a 2^-10 margin, and beyond X/4 (X = largest |coordinate| of i), see above
         const float xmax = fmaxf(fabsf(xh), fmaxf(fabsf(yh), fabsf(zh)));
         I[u].hfar2 = live ? fmaxf(I[u].h2 * 1.0009765625f, kFarFraction2 * xmax * xmax) : -1.f;
+        if (VEL) {
+            const float dtr = live ? fabsf(__double2float_rn(a.dtr[row])) : 0.f;
+            const float vi = sqrtf(vx * vx + vy * vy + vz * vz) * 1.000001f;
+            I[u].dtr = live ? __double2float_rn(a.dtr[row]) : 0.f;
+            I[u].hfar_x = live ? sqrtf(kFarFraction2) * xmax : 0.f;  // dead rows: hfar2 = 0, never near
+            I[u].hfar_r = live ? fmaf(dtr, vi, sqrtf(I[u].h2) * 1.00048828125f) : 0.f;
+        }
         I[u].self = i;
         I[u].nlim = (live && h2 >= 1.17549435e-38f) ? a.n : 0;
         I[u].cnt = 0;
@@ -276,7 +310,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         I[u].list = a.nbr_list + (size_t)row * a.cap;
         accum_zero(s[u]);
 #pragma unroll
-        for (int c = 0; c < 6; ++c) sum[u][c] = 0.0;
+        for (int c = 0; c < kSums; ++c) sum[u][c] = 0.0;
     }
 
     // ---- S3/S4: stream the j-tiles
@@ -290,6 +324,14 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         mbar_wait(&full[st], (lt >> 1) & 1);
         const float4* tp = tiles + st * kTileQuads;
         const int32_t jbase = (t_begin + lt) * JT;
+        if (VEL) {  // far threshold of this tile: its fastest particle cannot bring a far pair within r_s during dtr
+            const float vmax = __ldg(a.tile_vmax + (jbase >> 8));
+#pragma unroll
+            for (int u = 0; u < IPT; ++u) {
+                const float hf = fmaxf(I[u].hfar_x, fmaf(fabsf(I[u].dtr), vmax, I[u].hfar_r));
+                I[u].hfar2 = hf * hf;
+            }
+        }
 #pragma unroll 2
         for (int p = 0; p < JT / 2; ++p) {
             const float4 q0 = tp[p * 5 + 0], q1 = tp[p * 5 + 1], q2 = tp[p * 5 + 2];
@@ -308,8 +350,10 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
 #pragma unroll
                 for (int u = 0; u < IPT; ++u) {
                     geom_lo(xl, q4, I[u], g[u]);
-                    const bool nb0 = g[u].r2.x < I[u].h2;  // eq. (2)/(11): neighbour iff r^2 < r_s^2
-                    const bool nb1 = g[u].r2.y < I[u].h2;
+                    // eq. (2)/(11): neighbour iff r^2 < r_s^2; eq. (3): iff min(r^2, |R + dtr V|^2) < r_s^2
+                    const float2 rm = VEL ? rmin2_velocity(q2, vz, I[u], g[u]) : g[u].r2;
+                    const bool nb0 = rm.x < I[u].h2;
+                    const bool nb1 = rm.y < I[u].h2;
                     int32_t* shared_count = split ? a.slot_count + (rows[u] - tail_row0) : nullptr;
                     append(I[u], j, nb0, a.cap, shared_count);
                     append(I[u], j + 1, nb1, a.cap, shared_count);
@@ -318,7 +362,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
                 }
             }
 #pragma unroll
-            for (int u = 0; u < IPT; ++u) pair_sum(q1, q2, vz, I[u], g[u], s[u]);
+            for (int u = 0; u < IPT; ++u) pair_sum<POT>(q1, q2, vz, I[u], g[u], s[u]);
         }
         // ---- S6: flush the tile's fp32 partial sums into the fp64 running sums
 #pragma unroll
@@ -329,6 +373,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
             sum[u][3] += (double)s[u].jx.x + (double)s[u].jx.y;
             sum[u][4] += (double)s[u].jy.x + (double)s[u].jy.y;
             sum[u][5] += (double)s[u].jz.x + (double)s[u].jz.y;
+            if (POT) sum[u][kSums - 1] += (double)s[u].pot.x + (double)s[u].pot.y;
             accum_zero(s[u]);
         }
         if (WARPS > 1) __syncthreads(); else __syncwarp();  // every warp is done with stage st before it is refilled
@@ -345,14 +390,15 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
                 a.acc[row * 3 + c] = sum[u][c];
                 a.jerk[row * 3 + c] = sum[u][3 + c];
             }
+            if (POT) a.pot[row] = sum[u][kSums - 1];
             a.nbr_count[row] = I[u].cnt;
             if (I[u].cnt > a.cap) atomicAdd(a.overflow_ws, 1);
         } else {
             flush_pending(I[u], a.cap);
             const size_t pi = (size_t)(row - tail_row0) * a.n_chunks + chunk;
-            double* ps = a.part_sum + pi * 6;
+            double* ps = a.part_sum + pi * kSums;
 #pragma unroll
-            for (int c = 0; c < 6; ++c) ps[c] = sum[u][c];
+            for (int c = 0; c < kSums; ++c) ps[c] = sum[u][c];
         }
     }
 }

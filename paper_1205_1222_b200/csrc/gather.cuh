@@ -22,9 +22,10 @@ struct GatherArgs {
     int32_t n_chunks;
     int32_t chunk_j;           // j-particles per chunk (tiles_per_chunk * j-tile)
     int32_t cap;
-    const double* part_sum;    // [split rows][S][6]
+    const double* part_sum;    // [split rows][S][6], or [..][7] with the potential
     double* acc;
     double* jerk;
+    double* pot;               // null: no potential (6 partial sums per chunk), else 7
     int32_t* nbr_count;
     int32_t* nbr_list;
     int32_t* n_overflow;
@@ -47,17 +48,20 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
     const size_t rbase = (size_t)prow * S;
 
     // ---- partial sums (fixed order: chunk = lane, lane + 32, ...; then xor tree 16, 8, 4, 2, 1)
-    double s[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    double s[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    const int n_sums = a.pot ? 7 : 6;
     for (int c = lane; c < S; c += 32) {
-        const double* ps = a.part_sum + (rbase + c) * 6;
+        const double* ps = a.part_sum + (rbase + c) * n_sums;
 #pragma unroll
-        for (int k = 0; k < 6; ++k) s[k] += ps[k];
+        for (int k = 0; k < 7; ++k)
+            if (k < n_sums) s[k] += ps[k];
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
 #pragma unroll
-        for (int k = 0; k < 6; ++k) s[k] += __shfl_xor_sync(0xffffffffu, s[k], off);
+        for (int k = 0; k < 7; ++k) s[k] += __shfl_xor_sync(0xffffffffu, s[k], off);
     }
+    if (lane == 0 && a.pot) a.pot[row] = s[6];
     if (lane < 3) {
         a.acc[row * 3 + lane] = (lane == 0) ? s[0] : (lane == 1) ? s[1] : s[2];
         a.jerk[row * 3 + lane] = (lane == 0) ? s[3] : (lane == 1) ? s[4] : s[5];

@@ -61,14 +61,15 @@ struct Plan {
 struct WorkspaceLayout {
     size_t packed_off, packed_bytes;
     size_t psum_off, psum_bytes;
+    size_t vmax_off, vmax_bytes;   // float speed bound per 256 consecutive j (predictor -> velocity criterion)
     size_t slot_off, slot_bytes;   // int32 list-slot counters of the j-split rows (zero between calls)
     size_t ctl_off, ctl_bytes;     // int32 {overflow count, gather ticket} (zero between calls)
     int64_t row_chunk_limit;  // (row, j-chunk) slots of partial sums
     size_t total;
 };
 
-// The j-split workspace holds 6 doubles per (row, chunk): enough slots for 64 chunks per row of the largest
-// block, at least 131072 (small blocks are split hundreds of ways), at most 2M (96 MB).
+// The j-split workspace holds 7 doubles per (row, chunk): enough slots for 64 chunks per row of the largest
+// block, at least 131072 (small blocks are split hundreds of ways), at most 2M (112 MB).
 int64_t row_chunk_slots(int64_t n_i_max) {
     return std::min<int64_t>(std::max<int64_t>(64 * n_i_max, 131072), 2097152);
 }
@@ -85,7 +86,8 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
         off += (size_t)round_up((int64_t)bytes, 256);
     };
     place((size_t)n_pad * kBytesPerJ, w.packed_off, w.packed_bytes);
-    place((size_t)w.row_chunk_limit * 6 * sizeof(double), w.psum_off, w.psum_bytes);
+    place((size_t)w.row_chunk_limit * 7 * sizeof(double), w.psum_off, w.psum_bytes);  // acc, jerk, pot
+    place((size_t)(n_pad / kJPad) * sizeof(float), w.vmax_off, w.vmax_bytes);
     place((size_t)(n_i_max + 512) * sizeof(int32_t), w.slot_off, w.slot_bytes);
     place(64, w.ctl_off, w.ctl_bytes);
     w.total = off;
@@ -97,7 +99,7 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
 struct nb_ctx {
     int device = 0;
     int num_sms = 0;
-    int ctas_per_sm[kNumShapes] = {0, 0, 0, 0, 0};  // resident CTAs per SM of each force-kernel shape
+    int ctas_per_sm[4][kNumShapes] = {};  // resident CTAs per SM of each force-kernel variant and shape
     int64_t n_max = 0, n_i_max = 0;
     int32_t cap = 0;
     unsigned char* ws = nullptr;
@@ -226,27 +228,30 @@ size_t force_smem_bytes(int ipt, int warps, int jt) {
     return 2 * (size_t)jt * kBytesPerJ + 2 * sizeof(uint64_t);
 }
 
-template <int IPT, int WARPS, int JT, int MINB>
+template <int IPT, int WARPS, int JT, int MINB, bool VEL, bool POT>
 int query_force(int* per_sm) {
-    auto kern = force_kernel<IPT, WARPS, JT, MINB>;
+    auto kern = force_kernel<IPT, WARPS, JT, MINB, VEL, POT>;
     const size_t smem = force_smem_bytes(IPT, WARPS, JT);
     NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     NB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, WARPS * 32, smem));
     return NB_OK;
 }
 
-template <int IPT, int WARPS, int JT, int MINB>
+template <int IPT, int WARPS, int JT, int MINB, bool VEL, bool POT>
 int launch_force(const Plan& p, const ForceArgs& fa, cudaStream_t st) {
     const size_t smem = force_smem_bytes(IPT, WARPS, JT);
-    force_kernel<IPT, WARPS, JT, MINB><<<p.grid, WARPS * 32, smem, st>>>(fa);
+    force_kernel<IPT, WARPS, JT, MINB, VEL, POT><<<p.grid, WARPS * 32, smem, st>>>(fa);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }
 
-// one switch for both: keeps the template arguments of query and launch in one place
-int force_dispatch(int shape, int* per_sm, const Plan* p, const ForceArgs* fa, cudaStream_t st) {
-#define NB_SHAPE(IPT, WARPS, JT, MINB) \
-    (per_sm ? query_force<IPT, WARPS, JT, MINB>(per_sm) : launch_force<IPT, WARPS, JT, MINB>(*p, *fa, st))
+// one switch for both: keeps the template arguments of query and launch in one place.  variant: bit 0 = velocity
+// criterion eq. (3), bit 1 = potential output (the kernel variants of Listing B2)
+template <bool VEL, bool POT>
+int force_dispatch_v(int shape, int* per_sm, const Plan* p, const ForceArgs* fa, cudaStream_t st) {
+#define NB_SHAPE(IPT, WARPS, JT, MINB)                               \
+    (per_sm ? query_force<IPT, WARPS, JT, MINB, VEL, POT>(per_sm) \
+            : launch_force<IPT, WARPS, JT, MINB, VEL, POT>(*p, *fa, st))
     switch (shape) {
         case 0: return NB_SHAPE(1, 8, 256, NBREG_CTAS256);
         case 1: return NB_SHAPE(1, 4, 128, 2 * NBREG_CTAS256);
@@ -257,6 +262,15 @@ int force_dispatch(int shape, int* per_sm, const Plan* p, const ForceArgs* fa, c
 #undef NB_SHAPE
 }
 
+int force_dispatch(int variant, int shape, int* per_sm, const Plan* p, const ForceArgs* fa, cudaStream_t st) {
+    switch (variant & 3) {
+        case 0: return force_dispatch_v<false, false>(shape, per_sm, p, fa, st);
+        case 1: return force_dispatch_v<true, false>(shape, per_sm, p, fa, st);
+        case 2: return force_dispatch_v<false, true>(shape, per_sm, p, fa, st);
+        default: return force_dispatch_v<true, true>(shape, per_sm, p, fa, st);
+    }
+}
+
 int run_predict(nb_ctx* c, double t, cudaStream_t st, double* xp_out, double* vp_out) {
     PredictArgs pa{};
     pa.n = c->n;
@@ -264,6 +278,7 @@ int run_predict(nb_ctx* c, double t, cudaStream_t st, double* xp_out, double* vp
     pa.x0 = c->x0; pa.v0 = c->v0; pa.a0 = c->a0; pa.j0 = c->j0; pa.m = c->m; pa.t0 = c->t0;
     pa.t = t;
     pa.packed = reinterpret_cast<float4*>(c->ws + c->lay.packed_off);
+    pa.tile_vmax = reinterpret_cast<float*>(c->ws + c->lay.vmax_off);
     pa.xp_out = xp_out;
     pa.vp_out = vp_out;
     const int threads = 256;
@@ -325,11 +340,13 @@ int nb_create(nb_ctx** out, int device, int64_t n_max, int64_t n_i_max, int32_t 
         delete c;
         return cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(reduce_gather_kernel)");
     }
-    for (int k = 0; k < kNumShapes; ++k) {
-        const int rc = force_dispatch(k, &c->ctas_per_sm[k], nullptr, nullptr, nullptr);
-        if (rc != NB_OK) {
-            delete c;
-            return rc;
+    for (int v = 0; v < 4; ++v) {
+        for (int k = 0; k < kNumShapes; ++k) {
+            const int rc = force_dispatch(v, k, &c->ctas_per_sm[v][k], nullptr, nullptr, nullptr);
+            if (rc != NB_OK) {
+                delete c;
+                return rc;
+            }
         }
     }
     c->n_max = n_max;
@@ -404,6 +421,13 @@ int nb_get_predicted(nb_ctx* c, double* xp, double* vp, void* stream) {
 
 int nb_regular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const double* r_s, double t, double* acc,
                      double* jerk, int32_t* nbr_count, int32_t* nbr_list, int32_t* n_overflow, void* stream) {
+    return nb_regular_force_ex(c, n_i, i_idx, r_s, nullptr, t, acc, jerk, nullptr, nbr_count, nbr_list, n_overflow,
+                               stream);
+}
+
+int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const double* r_s, const double* dtr, double t,
+                        double* acc, double* jerk, double* pot, int32_t* nbr_count, int32_t* nbr_list,
+                        int32_t* n_overflow, void* stream) {
     if (!c || !n_overflow) return NB_E_INVAL;
     if (n_i < 0 || n_i > c->n_i_max) return NB_E_INVAL;
     if (n_i > 0 && (!i_idx || !r_s || !acc || !jerk || !nbr_count || !nbr_list)) return NB_E_INVAL;
@@ -425,7 +449,8 @@ int nb_regular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const double*
     mach.n = c->n;
     mach.row_chunk_limit = c->lay.row_chunk_limit;
     mach.num_sms = c->num_sms;
-    for (int k = 0; k < kNumShapes; ++k) mach.ctas_per_sm[k] = c->ctas_per_sm[k];
+    const int variant = (dtr ? 1 : 0) | (pot ? 2 : 0);
+    for (int k = 0; k < kNumShapes; ++k) mach.ctas_per_sm[k] = c->ctas_per_sm[variant][k];
     const Plan p = make_plan(&mach, n_i, c->opt_i_block, c->opt_j_split);
     ForceArgs fa{};
     fa.packed = reinterpret_cast<const float4*>(c->ws + c->lay.packed_off);
@@ -438,6 +463,9 @@ int nb_regular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const double*
     fa.cap = c->cap;
     fa.i_idx = i_idx;
     fa.r_s = r_s;
+    fa.dtr = dtr;
+    fa.tile_vmax = reinterpret_cast<const float*>(c->ws + c->lay.vmax_off);
+    fa.pot = pot;
     fa.acc = acc; fa.jerk = jerk; fa.nbr_count = nbr_count; fa.nbr_list = nbr_list; fa.n_overflow = n_overflow;
     fa.part_sum = reinterpret_cast<double*>(c->ws + c->lay.psum_off);
     const Shape& sh = kShapes[p.shape];
@@ -446,7 +474,7 @@ int nb_regular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const double*
     int32_t* ctl = reinterpret_cast<int32_t*>(c->ws + c->lay.ctl_off);
     fa.slot_count = reinterpret_cast<int32_t*>(c->ws + c->lay.slot_off);
     fa.overflow_ws = ctl;
-    int rc = force_dispatch(p.shape, nullptr, &p, &fa, st);
+    int rc = force_dispatch(variant, p.shape, nullptr, &p, &fa, st);
     if (rc != NB_OK) return rc;
     ++launches;
     {  // S5 + n_overflow: always launched, with no rows when nothing was split
@@ -454,7 +482,7 @@ int nb_regular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const double*
         ga.row0 = (int32_t)(has_split ? row0 : n_i); ga.n_i = n_i; ga.n_chunks = p.n_chunks; ga.cap = c->cap;
         ga.chunk_j = p.tiles_per_chunk * sh.jt;
         ga.part_sum = fa.part_sum;
-        ga.acc = acc; ga.jerk = jerk; ga.nbr_count = nbr_count; ga.nbr_list = nbr_list; ga.n_overflow = n_overflow;
+        ga.acc = acc; ga.jerk = jerk; ga.pot = pot; ga.nbr_count = nbr_count; ga.nbr_list = nbr_list; ga.n_overflow = n_overflow;
         ga.slot_count = fa.slot_count; ga.overflow_ws = ctl; ga.ticket = ctl + 1;
         const int64_t split_rows = has_split ? n_i - row0 : 0;
         const unsigned blocks = (unsigned)std::max<int64_t>(1, (split_rows + kGatherWarps - 1) / kGatherWarps);
@@ -465,7 +493,7 @@ int nb_regular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const double*
     }
     c->info[0] = sh.rows; c->info[1] = sh.ipt; c->info[2] = p.n_chunks; c->info[3] = p.grid;
     c->info[4] = p.n_blocks - p.main_blocks; c->info[5] = launches; c->info[6] = sh.jt;
-    c->info[7] = c->ctas_per_sm[p.shape];
+    c->info[7] = c->ctas_per_sm[variant][p.shape];
     return NB_OK;
 }
 

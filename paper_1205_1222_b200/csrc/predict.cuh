@@ -19,6 +19,7 @@ struct PredictArgs {
     const double* t0;
     double t;
     float4* packed;
+    float* tile_vmax;  // [n_pad / 256] upper bound of |v_p| over each block of 256 consecutive particles
     double* xp_out;  // fp64 outputs (test hook), used only when WRITE_F64
     double* vp_out;
 };
@@ -35,13 +36,20 @@ __device__ __forceinline__ void load3(const double* base, int64_t j, double (&ou
     out[off + 2] = __ldg(base + 3 * j + 2);
 }
 
+// The kernel also leaves, per block of 256 consecutive particles (= kJPad, a multiple of every j-tile), an upper
+// bound of the predicted speed: the velocity neighbour criterion eq. (3) needs |V_ij| bounded to
+// decide that a far pair cannot come within r_s during dtr (force.cuh).
 template <bool WRITE_F64>
 __global__ void __launch_bounds__(256) predict_kernel(PredictArgs a) {
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= a.n_pairs) return;
+    const bool active = p < a.n_pairs;
     const int64_t j0 = 2 * p;
     float xh[6], xl[6], vf[6], mf[2];
-    if (j0 >= a.n) {  // padding pair: massless, far away, at rest
+#pragma unroll
+    for (int k = 0; k < 6; ++k) vf[k] = 0.f;
+    if (!active) {
+        // nothing to predict; the thread still takes part in the speed reduction below
+    } else if (j0 >= a.n) {  // padding pair: massless, far away, at rest
 #pragma unroll
         for (int k = 0; k < 6; ++k) { xh[k] = kFarAway; xl[k] = 0.f; vf[k] = 0.f; }
         mf[0] = mf[1] = 0.f;
@@ -87,6 +95,21 @@ __global__ void __launch_bounds__(256) predict_kernel(PredictArgs a) {
         }
     }
     if (!WRITE_F64) {
+        // speed bound of this thread's pair, rounded up; max over the 128 threads (4 warps) of each 256-particle block
+        __shared__ float warp_max[8];
+        const float s0 = vf[0] * vf[0] + vf[1] * vf[1] + vf[2] * vf[2];
+        const float s1 = vf[3] * vf[3] + vf[4] * vf[4] + vf[5] * vf[5];
+        float vm = sqrtf(fmaxf(s0, s1)) * 1.000001f;
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) vm = fmaxf(vm, __shfl_xor_sync(0xffffffffu, vm, off));
+        if ((threadIdx.x & 31) == 0) warp_max[threadIdx.x >> 5] = vm;
+        __syncthreads();
+        if ((threadIdx.x & 127) == 0 && active) {
+            const int w = threadIdx.x >> 5;
+            a.tile_vmax[p >> 7] = fmaxf(fmaxf(warp_max[w], warp_max[w + 1]), fmaxf(warp_max[w + 2], warp_max[w + 3]));
+        }
+    }
+    if (!WRITE_F64 && active) {
         float4* o = a.packed + kQuadsPerPair * p;
         o[0] = make_float4(xh[0], xh[3], xh[1], xh[4]);
         o[1] = make_float4(xh[2], xh[5], mf[0], mf[1]);

@@ -7,7 +7,7 @@ import torch
 from paper_1205_1222_b200 import binding
 
 
-def run_gpu(wl, options=None, n_max=None, n_i_max=None, cap=None, ctx=None, want_pred=False):
+def run_gpu(wl, options=None, n_max=None, n_i_max=None, cap=None, ctx=None, want_pred=False, dtr=None, want_pot=False):
     """nb_create + nb_set_j + nb_regular_force (fused with the predictor) on cuda:0.  Returns (gpu dict of numpy
     arrays, launch info[, xp, vp])."""
     s = wl.state
@@ -23,7 +23,11 @@ def run_gpu(wl, options=None, n_max=None, n_i_max=None, cap=None, ctx=None, want
     r_s = torch.from_numpy(np.ascontiguousarray(wl.r_s, dtype=np.float64)).to(dev)
     out = ctx.alloc_outputs(wl.n_i)
     out["nbr_list"].fill_(-7)  # entries past the count must stay untouched
-    ctx.nb_regular_force(i_idx, r_s, s.t, out=out)
+    if dtr is None and not want_pot:
+        ctx.nb_regular_force(i_idx, r_s, s.t, out=out)
+    else:  # the Listing-B2 variants: velocity criterion eq. (3) and / or potential
+        dtr_t = None if dtr is None else torch.from_numpy(np.ascontiguousarray(dtr, dtype=np.float64)).to(dev)
+        ctx.nb_regular_force_ex(i_idx, r_s, s.t, dtr=dtr_t, want_pot=want_pot, out=out)
     torch.cuda.synchronize()
     info = ctx.nb_last_launch_info()
     gpu = {k: v.cpu().numpy() for k, v in out.items()}

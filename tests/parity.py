@@ -12,6 +12,7 @@ import numpy as np
 
 TOL_ACC = 1e-6
 TOL_JERK = 1e-5
+TOL_POT = 1e-6  # the potential is a sum of positive terms like acc's dominant part: same bound
 BAND = 1e-6
 
 
@@ -21,10 +22,20 @@ def relerr(a, b):
     return np.linalg.norm(a - b, axis=-1) / den
 
 
-def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None):
+def _rmin(xp, vp, i, j, dt):
+    """r_min of eq. (3) for the pairs (i, j): min(|R|, |R + dt V|); dt = 0 gives |R|."""
+    R = xp[j] - xp[i]
+    d = np.linalg.norm(R, axis=-1)
+    if dt != 0.0:
+        d = np.minimum(d, np.linalg.norm(R + dt * (vp[j] - vp[i]), axis=-1))
+    return d
+
+
+def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None, dtr=None, check_pot=False):
     """gpu: dict of numpy arrays acc, jerk, nbr_count, nbr_list, n_overflow (full block).
-    rows: optional subset of row numbers to check (oracle runs only on those).  Returns a report dict;
-    raises AssertionError on a violation."""
+    rows: optional subset of row numbers to check (oracle runs only on those).
+    dtr: per-row regular steps -> velocity criterion eq. (3) (band measured on r_min); check_pot: compare gpu["pot"].
+    Returns a report dict; raises AssertionError on a violation."""
     i_idx = np.asarray(i_idx)
     if rows is None:
         rows = np.arange(i_idx.shape[0])
@@ -32,7 +43,13 @@ def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None
     sub_idx = np.ascontiguousarray(i_idx[rows], dtype=np.int32)
     sub_rs = np.ascontiguousarray(r_s[rows])
     stride = list_stride or max(2 * cap, 64)
-    acc_o, jerk_o, cnt_o, lists_o = oracle.regular_force(xp, vp, m, sub_idx, sub_rs, list_stride=stride)
+    ex = dtr is not None or check_pot
+    sub_dt = np.zeros(rows.shape[0]) if dtr is None else np.ascontiguousarray(np.asarray(dtr)[rows], dtype=np.float64)
+    if ex:
+        acc_o, jerk_o, pot_o, cnt_o, lists_o = oracle.regular_force_ex(xp, vp, m, sub_idx, sub_rs,
+                                                                       None if dtr is None else sub_dt, list_stride=stride)
+    else:
+        acc_o, jerk_o, cnt_o, lists_o = oracle.regular_force(xp, vp, m, sub_idx, sub_rs, list_stride=stride)
     acc_g, jerk_g = gpu["acc"][rows].copy(), gpu["jerk"][rows].copy()
     cnt_g = gpu["nbr_count"][rows]
     list_g = gpu["nbr_list"][rows]
@@ -60,13 +77,13 @@ def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None
         i = sub_idx[q]
         if cnt_g[q] > cap and not diff:
             # counts differ on an overflowed row: cannot name the pair; bound the number of band pairs instead
-            d = np.linalg.norm(xp - xp[i], axis=1)
+            d = _rmin(xp, vp, i, np.arange(xp.shape[0]), sub_dt[q])
             nband = int((np.abs(d - sub_rs[q]) < BAND * sub_rs[q]).sum())
             assert abs(int(cnt_g[q]) - int(cnt_o[q])) <= nband, f"row {rows[q]}: overflow count mismatch"
             n_band_pairs += abs(int(cnt_g[q]) - int(cnt_o[q]))
             continue
         for j in diff:
-            d = np.linalg.norm(xp[j] - xp[i])
+            d = float(_rmin(xp, vp, i, j, sub_dt[q]))
             off = abs(d - sub_rs[q]) / sub_rs[q]
             assert off < BAND, f"row {rows[q]} (i={i}): list differs at j={j}, |r-r_s|/r_s={off:.3e} outside band"
             worst_band = max(worst_band, off)
@@ -78,6 +95,14 @@ def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None
         rq = np.array(recheck)
         a2, j2 = oracle.force_given_lists(xp, vp, m, sub_idx[rq], [list_g[q, : cnt_g[q]] for q in rq])
         acc_o[rq], jerk_o[rq] = a2, j2
+        if check_pot:  # the same re-summation for the potential: move the band pairs' m / r across
+            for q in recheck:
+                i = sub_idx[q]
+                so, sg = set(lists_o[q].tolist()), set(list_g[q, : cnt_g[q]].tolist())
+                for j in so - sg:  # oracle excluded it, the GPU summed it
+                    pot_o[q] += m[j] / np.linalg.norm(xp[j] - xp[i])
+                for j in sg - so:
+                    pot_o[q] -= m[j] / np.linalg.norm(xp[j] - xp[i])
     ea, ej = relerr(acc_g, acc_o), relerr(jerk_g, jerk_o)
     # rows where everything is a neighbour have acc = jerk = 0 exactly on both sides
     zero = (np.linalg.norm(acc_o, axis=1) == 0)
@@ -86,7 +111,16 @@ def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None
     worst_a = int(np.argmax(ea))
     assert ea.max() <= TOL_ACC, f"acc rel err {ea.max():.3e} at row {rows[worst_a]} > {TOL_ACC}"
     assert ej.max() <= TOL_JERK, f"jerk rel err {ej.max():.3e} at row {rows[int(np.argmax(ej))]} > {TOL_JERK}"
-    return dict(rows=int(rows.shape[0]), max_acc_err=float(ea.max()), max_jerk_err=float(ej.max()),
+    max_pot = 0.0
+    if check_pot:
+        pot_g = gpu["pot"][rows]
+        den = np.where(pot_o == 0.0, 1.0, np.abs(pot_o))
+        ep = np.abs(pot_g - pot_o) / den
+        if zero.any():
+            assert np.all(pot_g[zero] == 0)
+        assert ep.max() <= TOL_POT, f"pot rel err {ep.max():.3e} at row {rows[int(np.argmax(ep))]} > {TOL_POT}"
+        max_pot = float(ep.max())
+    return dict(max_pot_err=max_pot, rows=int(rows.shape[0]), max_acc_err=float(ea.max()), max_jerk_err=float(ej.max()),
                 median_acc_err=float(np.median(ea)), band_pairs=int(n_band_pairs), worst_band=float(worst_band),
                 overflow_rows=int(n_over), mean_count=float(cnt_o.mean()))
 

@@ -1,0 +1,83 @@
+"""The kernel variants of the paper's Listing B2 against the oracle (-m gpu): velocity neighbour
+criterion eq. (3) through nb_regular_force_ex(dtr) and the potential output (pot)."""
+import numpy as np
+import pytest
+
+from paper_1205_1222_b200 import inputs
+import parity
+from gpu_util import run_gpu
+
+pytestmark = pytest.mark.gpu
+
+
+def _regular_steps(wl, factor=8.0):
+    """Per-row regular time-step: `factor` times the particle's own block-step (regular steps are several
+    irregular steps long); exact powers of two."""
+    s = wl.state
+    return np.ascontiguousarray((s.t - s.t0[wl.i_idx]) * factor)
+
+
+@pytest.mark.parametrize("config", [1, 2])
+@pytest.mark.parametrize("variant", ["vel", "pot", "vel+pot"])
+def test_configs_1_2_variants(oracle, config, variant):
+    wl = inputs.make_workload(config, forces=oracle.total_force, predict=lambda s: oracle.predict_state(s)[0])
+    dtr = _regular_steps(wl) if "vel" in variant else None
+    gpu, info = run_gpu(wl, dtr=dtr, want_pot="pot" in variant)
+    xp, vp = oracle.predict_state(wl.state)
+    rep = parity.compare(oracle, xp, vp, wl.state.m, wl.i_idx, wl.r_s, wl.cap, gpu, dtr=dtr, check_pot="pot" in variant)
+    parity.check_overflow_flag(gpu, wl.cap)
+    if dtr is not None:  # the criterion adds approaching particles: more neighbours than the k of the calibration
+        assert rep["mean_count"] > wl.k + 0.5
+    print(config, variant, info, rep)
+
+
+def test_zero_dtr_equals_plain_criterion(oracle):
+    wl = inputs.make_custom(3000, 900, 24, 64, predict=lambda s: oracle.predict_state(s)[0])
+    ref, _ = run_gpu(wl)
+    g, _ = run_gpu(wl, dtr=np.zeros(wl.n_i), want_pot=True)
+    assert np.array_equal(g["nbr_count"], ref["nbr_count"])
+    for q in range(wl.n_i):
+        c = ref["nbr_count"][q]
+        assert np.array_equal(g["nbr_list"][q, :c], ref["nbr_list"][q, :c])
+    assert parity.relerr(g["acc"], ref["acc"]).max() < 5e-7 and parity.relerr(g["jerk"], ref["jerk"]).max() < 5e-6
+
+
+@pytest.mark.parametrize("i_block,j_split", [(32, 5), (128, 1), (256, 3), (512, 2), (0, 0)])
+def test_variants_every_shape_ragged(oracle, i_block, j_split):
+    wl = inputs.make_custom(2999, 777, 24, 64, masses="salpeter", predict=lambda s: oracle.predict_state(s)[0])
+    dtr = _regular_steps(wl, 4.0)
+    dtr[:5] = 0.0
+    dtr[5:9] = 0.5  # long steps: many fast approachers
+    gpu, info = run_gpu(wl, options={"i_block": i_block, "j_split": j_split}, dtr=dtr, want_pot=True)
+    xp, vp = oracle.predict_state(wl.state)
+    parity.compare(oracle, xp, vp, wl.state.m, wl.i_idx, wl.r_s, wl.cap, gpu, dtr=dtr, check_pot=True)
+    parity.check_overflow_flag(gpu, wl.cap)
+
+
+def test_config4_binaries_velocity_and_potential(oracle):
+    wl = inputs.make_workload(4, predict=lambda s: oracle.predict_state(s)[0])
+    dtr = np.minimum(_regular_steps(wl), 2.0 ** -5)  # binary members have tiny own steps; cap the rest at 1/32
+    gpu, info = run_gpu(wl, dtr=dtr, want_pot=True)
+    xp, vp = oracle.predict_state(wl.state)
+    rep = parity.compare(oracle, xp, vp, wl.state.m, wl.i_idx, wl.r_s, wl.cap, gpu, dtr=dtr, check_pot=True,
+                         list_stride=2048)
+    assert parity.check_overflow_flag(gpu, wl.cap) >= 40
+    print(info, rep)
+
+
+def test_config3_potential_energy(oracle):
+    """Full block, r_s = 0: sum m_i pot_i = -2 W; for the Plummer model in N-body units W ~ -1/2.
+    With r_s = 0 nothing is excluded, so the closest pairs go through the fp32 pair math: that is outside the
+    method's regime ("all close interactions are skipped") and only the potential is checked here."""
+    st = inputs.make_state(3)
+    n = st.n
+    wl = inputs.Workload(st, np.arange(n, dtype=np.int32), np.zeros(n), 0, 8)
+    gpu, info = run_gpu(wl, want_pot=True)
+    W = -0.5 * float((st.m * gpu["pot"]).sum())
+    assert abs(W + 0.5) < 0.02
+    assert np.all(gpu["nbr_count"] == 0)
+    xp, vp = oracle.predict_state(st)
+    rows = np.random.default_rng(3).choice(n, 2048, replace=False)
+    _, _, pot_o, cnt_o, _ = oracle.regular_force_ex(xp, vp, st.m, wl.i_idx[rows], wl.r_s[rows])
+    assert np.all(cnt_o == 0)
+    assert np.max(np.abs(gpu["pot"][rows] / pot_o - 1.0)) <= parity.TOL_POT
