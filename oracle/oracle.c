@@ -22,6 +22,10 @@
  *                            the potential sum "fo.pot += mrinv1": pot_i = sum m_j / r_ij over
  *                            the same non-neighbours as eq. (9) (sign as in the listing: positive).
  *
+ *   oracle_irregular_force   step (iv), eq. (7), (8): force and its time derivative from the
+ *                            members of a given neighbour list (the job of the paper's GPUIRR library,
+ *                            PAPER.md:130-140).  Same pair term as eq. (9), (10), summed over j in L_i.
+ *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC oracle.c -o liboracle.so -lm
  * (-ffp-contract=off: no FMA contraction, so the arithmetic is exactly what is written.)
  */
@@ -198,5 +202,45 @@ void oracle_regular_force_ex(int64_t n, const double* xp, const double* vp, cons
         }
         if (pot) pot[q] = phi;
         count[q] = cnt;
+    }
+}
+
+/* Irregular force, eq. (7), (8): for row q, i = i_idx[q],
+ *   acc = sum over j in L_q of m_j R_ij / r^3,   jerk = sum of m_j [V_ij / r^3 - 3 (R_ij . V_ij) R_ij / r^5],
+ * L_q = lists[q*list_stride .. + min(counts[q], list_stride)), summed in list order.  An entry equal to i (the
+ * paper's device lists may contain self) or coincident with i (r = 0) is skipped.
+ * acc_scale, jerk_scale [n_i] (may be NULL): sum of the NORMS of the terms, sum m/r^2 and
+ * sum m (|V|/r^3 + 3 |R.V|/r^4): the yardstick for the rounding error of a sum whose terms cancel. */
+void oracle_irregular_force(int64_t n, const double* xp, const double* vp, const double* m, int64_t n_i,
+                            const int32_t* i_idx, const int32_t* lists, const int32_t* counts, int64_t list_stride,
+                            double* acc, double* jerk, double* acc_scale, double* jerk_scale) {
+    (void)n;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t q = 0; q < n_i; ++q) {
+        int64_t i = i_idx[q];
+        int64_t len = counts[q] < list_stride ? counts[q] : list_stride;
+        double a[3] = {0.0, 0.0, 0.0}, jk[3] = {0.0, 0.0, 0.0}, sa = 0.0, sj = 0.0;
+        for (int64_t e = 0; e < len; ++e) {
+            int64_t j = lists[q * list_stride + e];
+            if (j == i) continue;
+            double R[3], V[3];
+            for (int c = 0; c < 3; ++c) {
+                R[c] = xp[3 * j + c] - xp[3 * i + c];
+                V[c] = vp[3 * j + c] - vp[3 * i + c];
+            }
+            double r2 = R[0] * R[0] + R[1] * R[1] + R[2] * R[2];
+            if (r2 == 0.0) continue;
+            pair_term(R, V, r2, m[j], a, jk);
+            double r = sqrt(r2), rv = R[0] * V[0] + R[1] * V[1] + R[2] * V[2];
+            double vn = sqrt(V[0] * V[0] + V[1] * V[1] + V[2] * V[2]);
+            sa += m[j] / r2;
+            sj += m[j] * (vn / (r2 * r) + 3.0 * fabs(rv) / (r2 * r2));
+        }
+        for (int c = 0; c < 3; ++c) {
+            acc[3 * q + c] = a[c];
+            jerk[3 * q + c] = jk[c];
+        }
+        if (acc_scale) acc_scale[q] = sa;
+        if (jerk_scale) jerk_scale[q] = sj;
     }
 }

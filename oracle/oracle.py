@@ -41,6 +41,8 @@ def _load():
                                                  _i32p, ctypes.c_int64, _f64p, _f64p]
         lib.oracle_regular_force_ex.argtypes = [ctypes.c_int64, _f64p, _f64p, _f64p, ctypes.c_int64, _i32p, _f64p,
                                                 _f64p, _f64p, _f64p, _f64p, _i32p, _i32p, ctypes.c_int64]
+        lib.oracle_irregular_force.argtypes = [ctypes.c_int64, _f64p, _f64p, _f64p, ctypes.c_int64, _i32p, _i32p, _i32p,
+                                               ctypes.c_int64, _f64p, _f64p, _f64p, _f64p]
         _lib = lib
     return _lib
 
@@ -152,6 +154,31 @@ def force_given_lists(xp, vp, m, i_idx, lists, counts=None):
     _load().oracle_force_given_lists(n, _p(xp), _p(vp), _p(m), n_i, _pi(i_idx), _pi(padded), _pi(counts), stride,
                                      _p(acc), _p(jerk))
     return acc, jerk
+
+
+def irregular_force(xp, vp, m, i_idx, lists, counts=None):
+    """eq. (7), (8): force and jerk from the members of the given lists (python list of index
+    arrays, or a padded 2-D int32 array + counts).  Returns acc, jerk, acc_scale, jerk_scale (sums of term norms)."""
+    xp, vp, m = map(_d, (xp, vp, m))
+    i_idx = np.ascontiguousarray(i_idx, dtype=np.int32)
+    n, n_i = xp.shape[0], i_idx.shape[0]
+    if counts is None:
+        counts = np.array([len(l) for l in lists], dtype=np.int32)
+        stride = max(1, int(counts.max()) if n_i else 1)
+        padded = np.zeros((n_i, stride), dtype=np.int32)
+        for q, l in enumerate(lists):
+            padded[q, : len(l)] = l
+    else:
+        padded = np.ascontiguousarray(lists, dtype=np.int32)
+        counts = np.ascontiguousarray(counts, dtype=np.int32)
+        stride = padded.shape[1]
+    acc = np.empty((n_i, 3))
+    jerk = np.empty((n_i, 3))
+    sa = np.empty(n_i)
+    sj = np.empty(n_i)
+    _load().oracle_irregular_force(n, _p(xp), _p(vp), _p(m), n_i, _pi(i_idx), _pi(padded), _pi(counts), stride,
+                                   _p(acc), _p(jerk), _p(sa), _p(sj))
+    return acc, jerk, sa, sj
 
 
 def total_force(x, v, m):

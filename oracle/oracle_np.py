@@ -69,3 +69,25 @@ def regular_force_ex(xp, vp, m, i_idx, r_s, dtr=None):
         lists.append(np.nonzero(nb)[0].astype(np.int32))
     count = np.array([len(l) for l in lists], dtype=np.int32)
     return acc, jerk, pot, count, lists
+
+
+def irregular_force(xp, vp, m, i_idx, lists):
+    """eq. (7), (8), from the equations: sums over the given neighbour lists."""
+    xp = np.asarray(xp, dtype=np.float64)
+    vp = np.asarray(vp, dtype=np.float64)
+    m = np.asarray(m, dtype=np.float64)
+    acc = np.zeros((len(i_idx), 3))
+    jerk = np.zeros((len(i_idx), 3))
+    for q, i in enumerate(i_idx):
+        js = np.asarray([j for j in lists[q] if j != i], dtype=np.int64)
+        if js.size == 0:
+            continue
+        R = xp[js] - xp[i]
+        V = vp[js] - vp[i]
+        r = np.linalg.norm(R, axis=1)
+        ok = r > 0
+        R, V, r, mj = R[ok], V[ok], r[ok], m[js][ok]
+        rv = np.einsum("jc,jc->j", R, V)
+        acc[q] = (mj[:, None] * R / r[:, None] ** 3).sum(axis=0)
+        jerk[q] = (mj[:, None] * (V / r[:, None] ** 3 - 3.0 * rv[:, None] * R / r[:, None] ** 5)).sum(axis=0)
+    return acc, jerk

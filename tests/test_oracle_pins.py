@@ -365,3 +365,54 @@ def test_ex_c_vs_numpy():
     a2, j2, p2, c2, l2 = oracle_np.regular_force_ex(x, v, m, ii, rs, dtr)
     assert _rel(a, a2).max() < 1e-13 and _rel(j, j2).max() < 1e-12 and np.abs(p / p2 - 1).max() < 1e-13
     assert np.array_equal(c, c2) and all(np.array_equal(p_, q_) for p_, q_ in zip(l, l2))
+
+
+# ================================================================ NEXT-2: irregular force eq. (7), (8)
+@pytest.mark.parametrize("impl", [oracle, oracle_np])
+def test_irregular_two_body_and_ring(impl):
+    g = GOLD["P1_two_body"]
+    xp = np.array([g["xi"], g["xj"]], dtype=float)
+    vp = np.array([g["vi"], g["vj"]], dtype=float)
+    m = np.array([7.0, g["mj"]])
+    res = impl.irregular_force(xp, vp, m, np.array([0], dtype=np.int32), [np.array([1, 0], dtype=np.int32)])
+    np.testing.assert_allclose(res[0][0], g["acc"], rtol=0, atol=1e-17)  # the self entry (0) is skipped
+    np.testing.assert_allclose(res[1][0], g["jerk"], rtol=0, atol=1e-17)
+    res = impl.irregular_force(xp, vp, m, np.array([0], dtype=np.int32), [np.array([], dtype=np.int32)])
+    assert np.all(res[0] == 0) and np.all(res[1] == 0)
+
+
+def test_irregular_plus_regular_is_total():
+    """eq. (7) + eq. (9) = total force, eq. (8) + eq. (10) = total jerk, for any r_s: the list
+    sum and the masked all-j sum are two different loops of the oracle."""
+    x, v, m = _plummer(600)
+    ii = np.arange(0, 600, 2, dtype=np.int32)
+    rs = inputs.kth_neighbour_distance(x, ii, 20, brute=True) * 1.0001
+    a_tot, j_tot, _, _ = oracle.regular_force(x, v, m, ii, np.zeros(len(ii)))
+    a_reg, j_reg, cnt, lists = oracle.regular_force(x, v, m, ii, rs)
+    a_irr, j_irr, sa, sj = oracle.irregular_force(x, v, m, ii, lists)
+    assert _rel(a_reg + a_irr, a_tot).max() < 1e-13 and _rel(j_reg + j_irr, j_tot).max() < 1e-12
+    # list = everybody else: the irregular sum alone is the total
+    everyone = [np.delete(np.arange(600, dtype=np.int32), i) for i in ii]
+    a_all, j_all, _, _ = oracle.irregular_force(x, v, m, ii, everyone)
+    assert _rel(a_all, a_tot).max() < 1e-13 and _rel(j_all, j_tot).max() < 1e-12
+    # the scales bound the results (triangle inequality) and are far from tight when terms cancel
+    assert np.all(np.linalg.norm(a_irr, axis=1) <= sa * (1 + 1e-12))
+    assert np.all(np.linalg.norm(j_irr, axis=1) <= sj * (1 + 1e-12))
+    # C vs numpy
+    a_np, j_np = oracle_np.irregular_force(x, v, m, ii, lists)
+    assert _rel(a_irr, a_np).max() < 1e-13 and _rel(j_irr, j_np).max() < 1e-12
+
+
+def test_irregular_padded_lists_and_stride():
+    x, v, m = _plummer(200)
+    ii = np.array([3, 50, 120], dtype=np.int32)
+    lists = [np.array([1, 2, 7], dtype=np.int32), np.array([], dtype=np.int32), np.arange(0, 60, dtype=np.int32)]
+    a, j, _, _ = oracle.irregular_force(x, v, m, ii, lists)
+    padded = np.full((3, 16), 199, dtype=np.int32)  # stride 16 < 60: row 2 is cut at the stride (overflowed row)
+    counts = np.array([3, 0, 60], dtype=np.int32)
+    for q, l in enumerate(lists):
+        padded[q, : min(len(l), 16)] = l[:16]
+    a2, j2, _, _ = oracle.irregular_force(x, v, m, ii, padded, counts)
+    assert np.array_equal(a[:2], a2[:2]) and np.array_equal(j[:2], j2[:2])
+    a3, _, _, _ = oracle.irregular_force(x, v, m, ii[2:], [np.arange(0, 16, dtype=np.int32)])
+    assert np.array_equal(a2[2], a3[0])
