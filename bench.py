@@ -230,6 +230,28 @@ def run_gpu_arm(args):
     n_over = int(out["n_overflow"].item())
     mean_cnt = float(out["nbr_count"].double().mean().item())
 
+    # ---- the step on the other side of the neighbour list: irregular force eq. (7), (8) over the
+    # lists the last step produced.  Reported beside the headline, not part of it.
+    irr = None
+    if not args.no_irregular:
+        irr_out = None
+        for _ in range(3):
+            irr_out = ctx.nb_irregular_force(i_idx, out["nbr_count"], out["nbr_list"], s.t, out=irr_out)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for _ in range(5):
+            ctx.nb_irregular_force(i_idx, out["nbr_count"], out["nbr_list"], s.t, out=irr_out)
+        ev[1].record()
+        torch.cuda.synchronize()
+        t_irr = ev[0].elapsed_time(ev[1]) / 5 / 1e3
+        irr_pairs = int(torch.clamp(out["nbr_count"], max=wl.cap).sum().item())
+        irr = {"kernel": "irregular_kernel", "pairs": irr_pairs, "ms": t_irr * 1e3,
+               "value": irr_pairs / t_irr / 1e9, "unit": UNIT, "bound": "l2-gather",
+               "gathered_gb_per_s": irr_pairs * 40 / t_irr / 1e9,
+               "note": "eq. (7), (8) over the neighbour lists of the last step; 40 B of packed record gathered per pair "
+                       "(L2-resident at this N); no measured L2 peak exists in MEASURED_PEAKS.json, so no fraction is given"}
+
     # ---- e2e: C-ABI call with HOST (pinned) buffers, copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -287,6 +309,7 @@ def run_gpu_arm(args):
                                "note": f"152 B/j algorithmic (112 read + 40 written), peak {peaks['src']} copy bandwidth"},
         "launch": info, "gpu_launches": int(info["launches"] + 1) * args.steps,
         "mean_neighbours": mean_cnt, "overflow_rows": n_over, "clocks": clocks, "e2e": e2e,
+        "next_irregular": irr,
     }
     if not args.no_cpu and world >= 1:
         cb, _ = cpu_baseline(wl, target_seconds=args.cpu_seconds)
@@ -306,6 +329,7 @@ def main():
     ap.add_argument("--n-i", type=int, default=None, help="active-block size (configs 1, 3, 5 only)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-irregular", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     args = ap.parse_args()
     if args.impl == "reference":

@@ -112,6 +112,22 @@ int nb_regular_force_ex(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const do
                         double t, double* acc, double* jerk, double* pot, int32_t* nbr_count, int32_t* nbr_list,
                         int32_t* n_overflow, void* stream);
 
+/* Step (iv), eq. (7), (8), PAPER.md:94-98 (the job of the paper's GPUIRR library): the IRREGULAR
+ * force and its time derivative of n_i active particles, summed over the members of their neighbour lists,
+ *   acc = sum_{j in L} m_j R_ij / r^3,   jerk = sum_{j in L} m_j [V_ij / r^3 - 3 (R_ij.V_ij) R_ij / r^5],
+ * on the state predicted to time t (if t differs from the last prediction, nb_predict_j(t) runs first on the same
+ * stream: all particles are predicted, the paper's PRED_ALL mode).  Coordinate differences are two-float
+ * (PAPER.md:138), pair arithmetic fp32, the sum fp64 over 32 fp32 lane sums.
+ *   i_idx:       dev int32[n_i]               0-based particle indices
+ *   nbr_count:   dev int32[n_i]               list lengths; min(count, list_stride) entries are used
+ *   nbr_list:    dev int32[n_i][list_stride]  e.g. the nbr_list / nbr_cap of nb_regular_force.  Entries equal to the
+ *                                             row's own particle, outside [0, n), or coincident with it are skipped
+ *   acc, jerk:   dev double[n_i][3]
+ * Enqueues one kernel (plus the predictor if needed) on `stream`. */
+int nb_irregular_force(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const int32_t* nbr_count,
+                       const int32_t* nbr_list, int32_t list_stride, double t, double* acc, double* jerk,
+                       void* stream);
+
 /* End-to-end convenience with HOST buffers: copies the j-state and the active block to device buffers the
  * context owns (allocated on first use, sized by n_max / n_i_max / nbr_cap), runs nb_set_j + nb_regular_force
  * on an internal stream, copies acc, jerk, nbr_count, nbr_list (n_i x nbr_cap) and n_overflow back and

@@ -209,8 +209,9 @@ void oracle_regular_force_ex(int64_t n, const double* xp, const double* vp, cons
  *   acc = sum over j in L_q of m_j R_ij / r^3,   jerk = sum of m_j [V_ij / r^3 - 3 (R_ij . V_ij) R_ij / r^5],
  * L_q = lists[q*list_stride .. + min(counts[q], list_stride)), summed in list order.  An entry equal to i (the
  * paper's device lists may contain self) or coincident with i (r = 0) is skipped.
- * acc_scale, jerk_scale [n_i] (may be NULL): sum of the NORMS of the terms, sum m/r^2 and
- * sum m (|V|/r^3 + 3 |R.V|/r^4): the yardstick for the rounding error of a sum whose terms cancel. */
+ * acc_scale, jerk_scale [n_i] (may be NULL): sums of the natural MAGNITUDES of the terms, sum m/r^2 and
+ * sum 4 m |V|/r^3 (= m (|V|/r^3 + 3 |R||V||R|/r^5): R.V is bounded by |R||V|, and a rounded evaluation of R.V errs
+ * in proportion to |R||V|, not to |R.V|): the yardstick for the rounding error of a sum whose terms cancel. */
 void oracle_irregular_force(int64_t n, const double* xp, const double* vp, const double* m, int64_t n_i,
                             const int32_t* i_idx, const int32_t* lists, const int32_t* counts, int64_t list_stride,
                             double* acc, double* jerk, double* acc_scale, double* jerk_scale) {
@@ -231,10 +232,10 @@ void oracle_irregular_force(int64_t n, const double* xp, const double* vp, const
             double r2 = R[0] * R[0] + R[1] * R[1] + R[2] * R[2];
             if (r2 == 0.0) continue;
             pair_term(R, V, r2, m[j], a, jk);
-            double r = sqrt(r2), rv = R[0] * V[0] + R[1] * V[1] + R[2] * V[2];
+            double r = sqrt(r2);
             double vn = sqrt(V[0] * V[0] + V[1] * V[1] + V[2] * V[2]);
             sa += m[j] / r2;
-            sj += m[j] * (vn / (r2 * r) + 3.0 * fabs(rv) / (r2 * r2));
+            sj += 4.0 * m[j] * vn / (r2 * r);
         }
         for (int c = 0; c < 3; ++c) {
             acc[3 * q + c] = a[c];

@@ -49,6 +49,7 @@ def load(build_if_missing: bool = True):
     lib.nb_get_predicted.argtypes = [vp, vp, vp, vp]
     lib.nb_regular_force.argtypes = [vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp, vp]
     lib.nb_regular_force_ex.argtypes = [vp, i32, vp, vp, vp, dbl, vp, vp, vp, vp, vp, vp, vp]
+    lib.nb_irregular_force.argtypes = [vp, i32, vp, vp, vp, i32, dbl, vp, vp, vp]
     lib.nb_regular_force_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp]
     lib.nb_set_option.argtypes = [vp, ctypes.c_char_p, i64]
     lib.nb_last_launch_info.argtypes = [vp, ctypes.POINTER(i64)]
@@ -179,6 +180,20 @@ class Context:
             _dev(out["pot"], torch.float64, "pot") if want_pot else null,
             _dev(out["nbr_count"], torch.int32, "nbr_count"), _dev(out["nbr_list"], torch.int32, "nbr_list"),
             _dev(out["n_overflow"], torch.int32, "n_overflow"), _stream_ptr(stream)))
+        return out
+
+    # -- nb_irregular_force: eq. (7), (8) over given neighbour lists
+    def nb_irregular_force(self, i_idx, nbr_count, nbr_list, t: float, out=None, stream=None):
+        n_i = int(i_idx.shape[0])
+        dev = self.workspace.device
+        if out is None:
+            out = dict(acc=torch.empty((n_i, 3), dtype=torch.float64, device=dev),
+                       jerk=torch.empty((n_i, 3), dtype=torch.float64, device=dev))
+        stride = int(nbr_list.shape[1]) if nbr_list.dim() == 2 else 1
+        _check(self.lib.nb_irregular_force(
+            self._h, n_i, _dev(i_idx, torch.int32, "i_idx"), _dev(nbr_count, torch.int32, "nbr_count"),
+            _dev(nbr_list, torch.int32, "nbr_list"), stride, float(t),
+            _dev(out["acc"], torch.float64, "acc"), _dev(out["jerk"], torch.float64, "jerk"), _stream_ptr(stream)))
         return out
 
     # -- nb_regular_force_host (all tensors on the CPU; pinned memory recommended)

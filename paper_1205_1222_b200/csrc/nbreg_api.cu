@@ -11,6 +11,7 @@
 
 #include "force.cuh"
 #include "gather.cuh"
+#include "irregular.cuh"
 #include "nbreg_common.cuh"
 #include "predict.cuh"
 
@@ -494,6 +495,33 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     c->info[0] = sh.rows; c->info[1] = sh.ipt; c->info[2] = p.n_chunks; c->info[3] = p.grid;
     c->info[4] = p.n_blocks - p.main_blocks; c->info[5] = launches; c->info[6] = sh.jt;
     c->info[7] = c->ctas_per_sm[variant][p.shape];
+    return NB_OK;
+}
+
+int nb_irregular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const int32_t* nbr_count,
+                       const int32_t* nbr_list, int32_t list_stride, double t, double* acc, double* jerk,
+                       void* stream) {
+    if (!c) return NB_E_INVAL;
+    if (n_i < 0 || n_i > c->n_i_max || list_stride < 1) return NB_E_INVAL;
+    if (n_i > 0 && (!i_idx || !nbr_count || !nbr_list || !acc || !jerk)) return NB_E_INVAL;
+    if (c->n < 1) return NB_E_STATE;
+    NB_CUDA(cudaSetDevice(c->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (!c->predicted || c->t_pred != t) {  // predict all particles first, same stream (the paper's PRED_ALL mode)
+        int rc = nb_predict_j(c, t, stream);
+        if (rc != NB_OK) return rc;
+    }
+    if (n_i == 0) return NB_OK;
+    IrregularArgs ia{};
+    ia.packed = reinterpret_cast<const float4*>(c->ws + c->lay.packed_off);
+    ia.n = (int32_t)c->n;
+    ia.n_i = n_i;
+    ia.list_stride = list_stride;
+    ia.i_idx = i_idx; ia.nbr_count = nbr_count; ia.nbr_list = nbr_list;
+    ia.acc = acc; ia.jerk = jerk;
+    const unsigned blocks = (unsigned)((n_i + kIrrWarps - 1) / kIrrWarps);
+    irregular_kernel<<<blocks, kIrrWarps * 32, 0, st>>>(ia);
+    NB_CUDA(cudaGetLastError());
     return NB_OK;
 }
 

@@ -1,0 +1,102 @@
+"""Irregular force eq. (7), (8) through nb_irregular_force against the oracle (-m gpu).
+
+Acceptance: the irregular sum has ~k terms that largely cancel, so the rounding error of the
+fp32 pair math is measured against the sum of the term norms the oracle returns:
+|d acc| <= 1e-6 * sum m/r^2 and |d jerk| <= 1e-6 * sum 4 m |V|/r^3 per row (each term carries <= ~5e-7 of its
+natural magnitude).  The chain regular -> list -> irregular is also closed: acc_reg + acc_irr = total force."""
+import numpy as np
+import pytest
+import torch
+
+from paper_1205_1222_b200 import binding, inputs
+import parity
+
+pytestmark = pytest.mark.gpu
+
+TOL_TERMS = 1e-6
+
+
+def _run_chain(wl, want_irr_rows=None):
+    """nb_regular_force, then nb_irregular_force on the lists it produced (all on the device)."""
+    s = wl.state
+    ctx = binding.Context(s.n, max(wl.n_i, 1), wl.cap)
+    ctx.set_state(s)
+    dev = ctx.workspace.device
+    i_idx = torch.from_numpy(np.ascontiguousarray(wl.i_idx, dtype=np.int32)).to(dev)
+    r_s = torch.from_numpy(np.ascontiguousarray(wl.r_s)).to(dev)
+    reg = ctx.nb_regular_force(i_idx, r_s, s.t)
+    irr = ctx.nb_irregular_force(i_idx, reg["nbr_count"], reg["nbr_list"], s.t)
+    torch.cuda.synchronize()
+    out = {k: v.cpu().numpy() for k, v in reg.items()}
+    out["acc_irr"], out["jerk_irr"] = irr["acc"].cpu().numpy(), irr["jerk"].cpu().numpy()
+    ctx.close()
+    return out
+
+
+def _check_irregular(oracle, xp, vp, m, i_idx, out, cap, rows=None):
+    rows = np.arange(len(i_idx)) if rows is None else rows
+    cnt = out["nbr_count"][rows]
+    a_o, j_o, sa, sj = oracle.irregular_force(xp, vp, m, i_idx[rows], out["nbr_list"][rows], np.minimum(cnt, cap))
+    da = np.linalg.norm(out["acc_irr"][rows] - a_o, axis=1)
+    dj = np.linalg.norm(out["jerk_irr"][rows] - j_o, axis=1)
+    ok = sa > 0
+    assert np.all(da[~ok] == 0) and np.all(dj[~ok] == 0)  # empty lists give exact zeros
+    ea, ej = da[ok] / sa[ok], dj[ok] / sj[ok]
+    assert ea.max() <= TOL_TERMS, f"acc: {ea.max():.3e} of the summed term norms"
+    assert ej.max() <= TOL_TERMS, f"jerk: {ej.max():.3e} of the summed term norms"
+    rel_a = da[ok] / np.linalg.norm(a_o[ok], axis=1)
+    return dict(rows=int(len(rows)), max_err_vs_terms=(float(ea.max()), float(ej.max())),
+                acc_rel_to_result=dict(median=float(np.median(rel_a)), p99=float(np.quantile(rel_a, 0.99)),
+                                       max=float(rel_a.max())))
+
+
+@pytest.mark.parametrize("config", [1, 2, 4])
+def test_chain_regular_then_irregular(oracle, config):
+    wl = inputs.make_workload(config, predict=lambda s: oracle.predict_state(s)[0])
+    out = _run_chain(wl)
+    xp, vp = oracle.predict_state(wl.state)
+    rep = _check_irregular(oracle, xp, vp, wl.state.m, wl.i_idx, out, wl.cap)
+    # eq. (7) + eq. (9) = total force (rows whose list overflowed have lost members: skip them)
+    full = out["nbr_count"] <= wl.cap
+    a_tot, j_tot, _, _ = oracle.regular_force(xp, vp, wl.state.m, wl.i_idx, np.zeros(wl.n_i), want_lists=False)
+    scale = np.linalg.norm(a_tot, axis=1) + np.linalg.norm(out["acc_irr"], axis=1)
+    err = np.linalg.norm(out["acc"] + out["acc_irr"] - a_tot, axis=1) / scale
+    assert err[full].max() < 2e-6
+    print(config, rep)
+
+
+def test_config5_sampled_and_edges(oracle):
+    wl = inputs.make_workload(5)
+    out = _run_chain(wl)
+    xp, vp = oracle.predict_state(wl.state)
+    rows = np.random.default_rng(11).choice(wl.n_i, 8192, replace=False)
+    print(_check_irregular(oracle, xp, vp, wl.state.m, wl.i_idx, out, wl.cap, rows=rows))
+
+
+def test_lists_with_self_garbage_and_empty_rows(oracle):
+    wl = inputs.make_custom(1500, 300, 16, 32, predict=lambda s: oracle.predict_state(s)[0])
+    s = wl.state
+    xp, vp = oracle.predict_state(s)
+    rng = np.random.default_rng(2)
+    stride = 40
+    lists = rng.integers(0, s.n, size=(wl.n_i, stride)).astype(np.int32)
+    counts = rng.integers(0, stride + 8, size=wl.n_i).astype(np.int32)  # some counts exceed the stride
+    counts[:4] = 0
+    lists[4:8, 0] = wl.i_idx[4:8]     # self in the list: skipped
+    lists[8, 1] = -5                  # out of range: ignored
+    lists[9, 2] = s.n + 3
+    ctx = binding.Context(s.n, wl.n_i, 32)
+    ctx.set_state(s)
+    dev = ctx.workspace.device
+    irr = ctx.nb_irregular_force(torch.from_numpy(wl.i_idx).to(dev), torch.from_numpy(counts).to(dev),
+                                 torch.from_numpy(lists).to(dev), s.t)
+    torch.cuda.synchronize()
+    clean = [np.array([j for j in lists[q, : min(counts[q], stride)] if 0 <= j < s.n], dtype=np.int32)
+             for q in range(wl.n_i)]
+    a_o, j_o, sa, sj = oracle.irregular_force(xp, vp, s.m, wl.i_idx, clean)
+    a_g, j_g = irr["acc"].cpu().numpy(), irr["jerk"].cpu().numpy()
+    assert np.all(a_g[:4] == 0) and np.all(j_g[:4] == 0)
+    ok = sa > 0
+    assert (np.linalg.norm(a_g - a_o, axis=1)[ok] / sa[ok]).max() <= TOL_TERMS
+    assert (np.linalg.norm(j_g - j_o, axis=1)[ok] / sj[ok]).max() <= TOL_TERMS
+    ctx.close()
