@@ -306,7 +306,10 @@ def run_gpu_arm(args):
         "roofline_predictor": {"bound": "hbm", "kernel": "predict_kernel", "achieved": pred_bytes / t_pred / 1e9,
                                "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": pred_bytes / t_pred / 1e9 / peaks["hbm_gbs"],
                                "traffic": None, "ms": t_pred * 1e3,
-                               "note": f"152 B/j algorithmic (112 read + 40 written), peak {peaks['src']} copy bandwidth"},
+                               "note": f"152 B/j algorithmic (112 read + 40 written), peak {peaks['src']} copy bandwidth; ms is the "
+                                       f"interval between two events around ONE launch inside the step and includes the "
+                                       f"event-to-kernel latency (the kernel alone: 23.8 us = 6.7 TB/s in "
+                                       f"profiles/r1_bench_c5_launches.md)"},
         "launch": info, "gpu_launches": int(info["launches"] + 1) * args.steps,
         "mean_neighbours": mean_cnt, "overflow_rows": n_over, "clocks": clocks, "e2e": e2e,
         "next_irregular": irr,
