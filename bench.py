@@ -173,6 +173,52 @@ def workload_config(wl, config):
                   "(lists N_i x cap x 4 B), larger than the 126 MB L2 for the default workload"}
 
 
+def run_sweep(args):
+    """SURVEY 8(d) protocol for config 3: one row per active-block size 32 ... 65536 (us per call and Gpairs/s),
+    for nb_regular_force alone and for the fused call (predictor + force).  Prints one JSON line."""
+    import torch
+    from paper_1205_1222_b200 import binding, inputs
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the regular-force path has no CPU fallback)")
+    full = inputs.make_workload(3)
+    s = full.state
+    ctx = binding.Context(s.n, full.n_i, full.cap)
+    state_dev = ctx.set_state(s)
+    dev = ctx.workspace.device
+    rows = []
+    for n_i in inputs.CONFIG3_BLOCKS:
+        i_idx = torch.from_numpy(full.i_idx[:n_i].copy()).to(dev)
+        r_s = torch.from_numpy(full.r_s[:n_i].copy()).to(dev)
+        out = ctx.alloc_outputs(n_i)
+        ctx.nb_predict_j(s.t)
+        for _ in range(3):
+            ctx.nb_regular_force(i_idx, r_s, s.t, out=out)
+        reps = 20 if n_i >= 8192 else 200
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for _ in range(reps):
+            ctx.nb_regular_force(i_idx, r_s, s.t, out=out)
+        ev[1].record()
+        torch.cuda.synchronize()
+        ev[2].record()
+        for _ in range(reps):
+            ctx.nb_set_j(*state_dev)                       # invalidates the prediction: the next call is fused
+            ctx.nb_regular_force(i_idx, r_s, s.t, out=out)
+        ev[3].record()
+        torch.cuda.synchronize()
+        us = ev[0].elapsed_time(ev[1]) / reps * 1e3
+        us_fused = ev[2].elapsed_time(ev[3]) / reps * 1e3
+        info = ctx.nb_last_launch_info()
+        rows.append({"n_i": n_i, "us_per_call": us, "gpairs": n_i * s.n / us / 1e3, "us_fused": us_fused,
+                     "rows_per_cta": info["rows_per_cta"], "j_chunks": info["j_chunks"], "ctas": info["ctas"]})
+    print(json.dumps({"metric": METRIC, "unit": UNIT, "config": {"workload": "BASELINE.json configs[2] block sweep",
+                                                                 "n": s.n, "timing": "back-to-back calls between two events"},
+                      "sweep": rows}))
+    return 0
+
+
 def run_gpu_arm(args):
     import torch
     from paper_1205_1222_b200 import binding
@@ -333,10 +379,13 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-irregular", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="config 3 active-block sweep 32 ... 65536 (one JSON line)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
     return run_gpu_arm(args)
 
 

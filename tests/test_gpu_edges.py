@@ -158,3 +158,20 @@ def test_error_codes_on_device():
     with pytest.raises(binding.NbregError):
         ctx.nb_set_option("no_such_option", 1)
     ctx.close()
+
+
+def test_large_cap_and_overflow_on_every_path(oracle):
+    """cap = 2048 with lists of ~1000 entries (sort of long j-split rows), and overflow on rows that one CTA owns
+    (j_split = 1) as well as on j-split rows."""
+    wl = _wl(oracle, 1800, 96, 16, 2048)
+    wl.r_s[:6] = 1e3            # everything a neighbour: 1799 entries, fits cap 2048
+    wl.r_s[6:12] *= 4.0         # ~1000 neighbours
+    for opts in ({"j_split": 1}, {"i_block": 32, "j_split": 7}, {}):
+        gpu, _ = run_gpu(wl, options=opts)
+        _full_check(oracle, wl, gpu)
+        assert np.all(gpu["nbr_count"][:6] == wl.state.n - 1) and int(gpu["n_overflow"][0]) == 0
+    small = inputs.Workload(wl.state, wl.i_idx, wl.r_s, wl.k, 64)
+    for opts in ({"j_split": 1}, {"i_block": 64, "j_split": 5}):
+        gpu, _ = run_gpu(small, options=opts)
+        _full_check(oracle, small, gpu, cap=64)
+        assert int(gpu["n_overflow"][0]) >= 12
