@@ -130,4 +130,69 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
     }
 }
 
+// The same job with one BLOCK per row, for rows split into many chunks (small active blocks: hundreds of chunks per
+// row and few rows, so a warp per row would leave the machine empty and walk the chunks serially).
+//   Sums: the 128 threads stride over the chunks, xor-shuffle tree per warp, then the four warp sums are added in
+//   warp order: fixed order, deterministic.
+//   List: ascending j is plain ascending VALUE, and a row holds few entries compared with its chunks, so each
+//   thread ranks one entry against the staged row (rank = number of smaller entries; entries are distinct) and
+//   stores it at its rank: O(count^2 / 128) instead of O(chunks).
+constexpr int kWideThreads = 128;
+
+__global__ void __launch_bounds__(kWideThreads) reduce_gather_wide_kernel(GatherArgs a) {
+    extern __shared__ int32_t stage[];  // cap entries
+    __shared__ double warp_sum[kWideThreads / 32][7];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t prow = blockIdx.x;
+    const int64_t row = a.row0 + prow;  // grid = split rows exactly
+    const int S = a.n_chunks;
+    const size_t rbase = (size_t)prow * S;
+
+    double s[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    const int n_sums = a.pot ? 7 : 6;
+    for (int c = tid; c < S; c += kWideThreads) {
+        const double* ps = a.part_sum + (rbase + c) * n_sums;
+#pragma unroll
+        for (int k = 0; k < 7; ++k)
+            if (k < n_sums) s[k] += ps[k];
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) s[k] += __shfl_xor_sync(0xffffffffu, s[k], off);
+    }
+    if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) warp_sum[warp][k] = s[k];
+    }
+    const int32_t cnt = a.slot_count[prow];  // true count, may exceed cap
+    const int32_t stored = min(cnt, a.cap);
+    int32_t* out = a.nbr_list + (size_t)row * a.cap;
+    for (int32_t e = tid; e < stored; e += kWideThreads) stage[e] = out[e];
+    __syncthreads();
+    if (tid < 7 && tid < n_sums) {
+        const double v = ((warp_sum[0][tid] + warp_sum[1][tid]) + warp_sum[2][tid]) + warp_sum[3][tid];
+        if (tid < 3) a.acc[row * 3 + tid] = v;
+        else if (tid < 6) a.jerk[row * 3 + tid - 3] = v;
+        else a.pot[row] = v;
+    }
+    for (int32_t e = tid; e < stored; e += kWideThreads) {
+        const int32_t v = stage[e];
+        int32_t rank = 0;
+        for (int32_t k = 0; k < stored; ++k) rank += stage[k] < v;  // broadcast reads
+        out[rank] = v;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        a.nbr_count[row] = cnt;
+        a.slot_count[prow] = 0;
+        if (cnt > a.cap) atomicAdd(a.overflow_ws, 1);
+        __threadfence();
+        if (atomicAdd(a.ticket, 1) == (int32_t)gridDim.x - 1) {
+            *a.n_overflow = atomicExch(a.overflow_ws, 0);
+            *a.ticket = 0;
+        }
+    }
+}
+
 }  // namespace nbreg

@@ -130,6 +130,7 @@ namespace {
 // are split S ways along j.  Measured on B200 (profiles/, planner calibration): G equal CTAs
 // of duration t on `slots` slots take about w t + 0.2 t, w between G / slots and its ceiling; the last term is the
 // ragged end, which is why several waves of short CTAs beat one wave of long ones.
+constexpr int kWideGatherChunks = 64;  // rows split into more chunks than this are gathered by a block each
 constexpr double kPrologueJ = 48.0;
 constexpr double kRaggedEnd = 0.2;
 
@@ -341,6 +342,11 @@ int nb_create(nb_ctx** out, int device, int64_t n_max, int64_t n_i_max, int32_t 
         delete c;
         return cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(reduce_gather_kernel)");
     }
+    if (cudaFuncSetAttribute(reduce_gather_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)((size_t)nbr_cap * sizeof(int32_t))) != cudaSuccess) {
+        delete c;
+        return cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(reduce_gather_wide_kernel)");
+    }
     for (int v = 0; v < 4; ++v) {
         for (int k = 0; k < kNumShapes; ++k) {
             const int rc = force_dispatch(v, k, &c->ctas_per_sm[v][k], nullptr, nullptr, nullptr);
@@ -487,8 +493,12 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         ga.slot_count = fa.slot_count; ga.overflow_ws = ctl; ga.ticket = ctl + 1;
         const int64_t split_rows = has_split ? n_i - row0 : 0;
         const unsigned blocks = (unsigned)std::max<int64_t>(1, (split_rows + kGatherWarps - 1) / kGatherWarps);
-        const size_t stage = (size_t)kGatherWarps * (c->cap + p.n_chunks) * sizeof(int32_t);
-        reduce_gather_kernel<<<blocks, kGatherWarps * 32, stage, st>>>(ga);
+        if (has_split && p.n_chunks > kWideGatherChunks) {  // many chunks per row: one block per row
+            reduce_gather_wide_kernel<<<(unsigned)split_rows, kWideThreads, (size_t)c->cap * sizeof(int32_t), st>>>(ga);
+        } else {
+            const size_t stage = (size_t)kGatherWarps * (c->cap + p.n_chunks) * sizeof(int32_t);
+            reduce_gather_kernel<<<blocks, kGatherWarps * 32, stage, st>>>(ga);
+        }
         NB_CUDA(cudaGetLastError());
         ++launches;
     }
