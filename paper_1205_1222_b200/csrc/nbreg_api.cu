@@ -130,7 +130,10 @@ namespace {
 // are split S ways along j.  Measured on B200 (profiles/, planner calibration): G equal CTAs
 // of duration t on `slots` slots take about w t + 0.2 t, w between G / slots and its ceiling; the last term is the
 // ragged end, which is why several waves of short CTAs beat one wave of long ones.
-constexpr int kWideGatherChunks = 64;  // rows split into more chunks than this are gathered by a block each
+// rows split into more than kWideGatherChunks chunks are gathered by a block each, if there are few enough of them
+// that a warp per row would leave SMs idle
+constexpr int kWideGatherChunks = 64;
+constexpr int64_t kWideGatherRows = 4096;
 constexpr double kPrologueJ = 48.0;
 constexpr double kRaggedEnd = 0.2;
 
@@ -493,7 +496,7 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         ga.slot_count = fa.slot_count; ga.overflow_ws = ctl; ga.ticket = ctl + 1;
         const int64_t split_rows = has_split ? n_i - row0 : 0;
         const unsigned blocks = (unsigned)std::max<int64_t>(1, (split_rows + kGatherWarps - 1) / kGatherWarps);
-        if (has_split && p.n_chunks > kWideGatherChunks) {  // many chunks per row: one block per row
+        if (has_split && p.n_chunks > kWideGatherChunks && split_rows <= kWideGatherRows) {  // few rows, many chunks
             reduce_gather_wide_kernel<<<(unsigned)split_rows, kWideThreads, (size_t)c->cap * sizeof(int32_t), st>>>(ga);
         } else {
             const size_t stage = (size_t)kGatherWarps * (c->cap + p.n_chunks) * sizeof(int32_t);
