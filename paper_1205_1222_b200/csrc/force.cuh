@@ -176,16 +176,34 @@ __device__ __forceinline__ void geom_lo(const float2& xl, const float4& q4, cons
 
 // eq. (9), (10) for the two pairs: 3 FADD2 (V), 3 (R.V), 2 (m/r^3), 2 (alpha), 9 FFMA2 (sums); 2 MUFU.RSQ + 2 MUFU.RCP.
 // POT adds one packed add: pot += m ri (Listing B2: "fo.pot += mrinv1").
-template <bool POT>
+// REFINE (near path only): one Newton step on the MUFU results, rsqrt to ~0.5 ulp and rcp likewise.  The pairs of the
+// near path are the closest ones a row sums, i.e. the largest jerk terms, whose rounding decides how close a row
+// whose terms cancel can stay to the fp64 result; the common path pays nothing for it.
+// The caller passes r^2 = +inf for a masked (neighbour) pair: rsqrt and rcp give 0 and the Newton residuals are
+// formed so that no inf * 0 arises (the masked r^2 is replaced by 1 and the pair's mass by 0).
+template <bool POT, bool REFINE>
 __device__ __forceinline__ void pair_sum(const float4& q1, const float4& q2, const float2& vz, const IState& I,
                                          const PairGeom& g, Accum& s) {
     const float2 dvx = __fadd2_rn(make_float2(q2.x, q2.y), bc(I.nvx));
     const float2 dvy = __fadd2_rn(make_float2(q2.z, q2.w), bc(I.nvy));
     const float2 dvz = __fadd2_rn(vz, bc(I.nvz));
     const float2 rv = __ffma2_rn(g.dz, dvz, __ffma2_rn(g.dy, dvy, __fmul2_rn(g.dx, dvx)));
-    const float2 ri = make_float2(rsqrt_approx(g.r2.x), rsqrt_approx(g.r2.y));
-    const float2 ri2 = make_float2(rcp_approx(g.r2.x), rcp_approx(g.r2.y));
-    const float2 mri = __fmul2_rn(make_float2(q1.z, q1.w), ri);
+    float2 ri, ri2, mj = make_float2(q1.z, q1.w);
+    if (REFINE) {
+        const float inf = __int_as_float(0x7f800000);
+        const float2 x = make_float2(g.r2.x == inf ? 1.f : g.r2.x, g.r2.y == inf ? 1.f : g.r2.y);
+        mj = make_float2(g.r2.x == inf ? 0.f : mj.x, g.r2.y == inf ? 0.f : mj.y);
+        const float2 y0 = make_float2(rsqrt_approx(x.x), rsqrt_approx(x.y));
+        const float2 z0 = make_float2(rcp_approx(x.x), rcp_approx(x.y));
+        const float2 ey = __ffma2_rn(__fmul2_rn(x, y0), make_float2(-y0.x, -y0.y), bc(1.f));  // 1 - x y0^2
+        ri = __ffma2_rn(__fmul2_rn(y0, bc(0.5f)), ey, y0);                                      // y0 + y0 e / 2
+        const float2 ez = __ffma2_rn(x, make_float2(-z0.x, -z0.y), bc(1.f));                    // 1 - x z0
+        ri2 = __ffma2_rn(z0, ez, z0);                                                           // z0 + z0 e
+    } else {
+        ri = make_float2(rsqrt_approx(g.r2.x), rsqrt_approx(g.r2.y));
+        ri2 = make_float2(rcp_approx(g.r2.x), rcp_approx(g.r2.y));
+    }
+    const float2 mri = __fmul2_rn(mj, ri);
     const float2 mri3 = __fmul2_rn(mri, ri2);
     if (POT) s.pot = __fadd2_rn(s.pot, mri);
     const float2 al = __fmul2_rn(__fmul2_rn(rv, ri2), bc(-3.f));
@@ -359,10 +377,12 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
                     append(I[u], j + 1, nb1, a.cap, shared_count);
                     if (nb0) g[u].r2.x = __int_as_float(0x7f800000);
                     if (nb1) g[u].r2.y = __int_as_float(0x7f800000);
+                    pair_sum<POT, true>(q1, q2, vz, I[u], g[u], s[u]);
                 }
+                continue;  // the near path finishes the pair itself: nothing flows back into the common path
             }
 #pragma unroll
-            for (int u = 0; u < IPT; ++u) pair_sum<POT>(q1, q2, vz, I[u], g[u], s[u]);
+            for (int u = 0; u < IPT; ++u) pair_sum<POT, false>(q1, q2, vz, I[u], g[u], s[u]);
         }
         // ---- S6: flush the tile's fp32 partial sums into the fp64 running sums
 #pragma unroll

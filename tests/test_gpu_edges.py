@@ -46,11 +46,16 @@ def test_shapes_and_splits_agree_bitwise_on_lists_and_closely_on_sums(oracle):
         assert parity.relerr(g["acc"], ref["acc"]).max() < 5e-7
 
 
-@pytest.mark.parametrize("i_block", [32, 0])
+@pytest.mark.parametrize("i_block", [32, 256])
 def test_main_blocks_plus_split_tail(oracle, i_block):
     """More row blocks than CTA slots: whole waves run unsplit, the remaining blocks are j-split (atomic list
-    slots + rank sort in the gather kernel).  Rows are drawn with replacement so that N stays small."""
-    wl = _wl(oracle, 3001, 120001 if i_block else 250007, 24, 64)
+    slots + ordering in the gather kernel).  Rows are drawn with replacement so that N stays small."""
+    probe = _wl(oracle, 3001, 64, 24, 64)
+    _, info0 = run_gpu(probe, options={"i_block": i_block})
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    slots = sms * info0["ctas_per_sm"]
+    n_i = (slots + slots // 16) * i_block + 1  # one full wave of row blocks plus a 1/16 wave that must be split
+    wl = _wl(oracle, 3001, n_i, 24, 64)
     gpu, info = run_gpu(wl, options={"i_block": i_block})
     n_blocks = -(-wl.n_i // info["rows_per_cta"])
     assert 0 < info["split_row_blocks"] < n_blocks and info["j_chunks"] > 1
