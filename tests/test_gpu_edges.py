@@ -180,3 +180,26 @@ def test_large_cap_and_overflow_on_every_path(oracle):
         gpu, _ = run_gpu(small, options=opts)
         _full_check(oracle, small, gpu, cap=64)
         assert int(gpu["n_overflow"][0]) >= 12
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_seeded_random_shapes(oracle, seed):
+    """Seeded random sizes, caps, radii scales, CTA shapes, splits and variants against the oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    n = int(rng.integers(3, 6000))
+    n_i = int(rng.integers(1, 1500))
+    k = int(min(rng.integers(0, 60), n - 1))
+    cap = int(rng.choice([8, 32, 64, 200]))
+    wl = _wl(oracle, n, n_i, k, cap, masses=str(rng.choice(["equal", "salpeter"])), seed_sub=2 + seed)
+    wl.r_s *= rng.choice([0.5, 1.0, 1.0, 1.7], size=wl.n_i)       # some lists overflow small caps
+    wl.r_s[rng.random(wl.n_i) < 0.03] = 0.0
+    opts = {"i_block": int(rng.choice([0, 0, 32, 64, 128, 256, 512])), "j_split": int(rng.choice([0, 0, 1, 2, 9]))}
+    use_vel, use_pot = bool(rng.integers(0, 2)), bool(rng.integers(0, 2))
+    dtr = (wl.state.t - wl.state.t0[wl.i_idx]) * float(rng.choice([1.0, 8.0])) if use_vel else None
+    gpu, info = run_gpu(wl, options=opts, dtr=dtr, want_pot=use_pot)
+    xp, vp = oracle.predict_state(wl.state)
+    parity.compare(oracle, xp, vp, wl.state.m, wl.i_idx, wl.r_s, cap, gpu, dtr=dtr, check_pot=use_pot,
+                   list_stride=max(2 * cap, 512))
+    parity.check_overflow_flag(gpu, cap)
+    live = np.arange(cap)[None, :] < np.minimum(gpu["nbr_count"], cap)[:, None]
+    assert np.all(gpu["nbr_list"][~live] == -7)  # nothing written past the count
