@@ -17,6 +17,8 @@
  *   - [n][3] arrays are row-major (x, y, z contiguous per particle).  Indices are 0-based int32.
  *   - Every function returns NB_OK (0) or a negative NB_E_* code; on error nothing has been enqueued.
  *     nb_strerror() gives the text; for NB_E_CUDA it includes the CUDA error string of the last failure.
+ *   - A context is not thread-safe and owns ONE workspace: issue its calls from one thread at a time and keep them
+ *     on one stream (or order streams yourself); use one context per concurrent stream.
  *   - There is no CPU fallback: without a CUDA device every compute call fails with NB_E_CUDA.
  */
 #ifndef NBREG_H_

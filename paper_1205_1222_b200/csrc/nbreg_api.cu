@@ -340,13 +340,14 @@ int nb_create(nb_ctx** out, int device, int64_t n_max, int64_t n_i_max, int32_t 
     if (!c) return NB_E_NOMEM;
     c->device = device;
     cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
+    // function attributes are per process, not per context: allow the largest list capacity any context may ask for
     if (cudaFuncSetAttribute(reduce_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)((size_t)kGatherWarps * (nbr_cap + kMaxChunks) * sizeof(int32_t))) != cudaSuccess) {
+                             (int)((size_t)kGatherWarps * (kMaxNbrCap + kMaxChunks) * sizeof(int32_t))) != cudaSuccess) {
         delete c;
         return cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(reduce_gather_kernel)");
     }
     if (cudaFuncSetAttribute(reduce_gather_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)((size_t)nbr_cap * sizeof(int32_t))) != cudaSuccess) {
+                             (int)((size_t)kMaxNbrCap * sizeof(int32_t))) != cudaSuccess) {
         delete c;
         return cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(reduce_gather_wide_kernel)");
     }

@@ -203,3 +203,17 @@ def test_seeded_random_shapes(oracle, seed):
     parity.check_overflow_flag(gpu, cap)
     live = np.arange(cap)[None, :] < np.minimum(gpu["nbr_count"], cap)[:, None]
     assert np.all(gpu["nbr_list"][~live] == -7)  # nothing written past the count
+
+
+def test_two_contexts_with_different_caps(oracle):
+    """Kernel function attributes are per process: creating a second context with a small cap must not shrink what
+    the first one may launch (its gather kernel stages cap entries per row in shared memory)."""
+    big = _wl(oracle, 1500, 200, 16, 4096)
+    big.r_s[:4] = 1e3
+    ctx_big = binding.Context(big.state.n, big.n_i, big.cap)
+    ctx_small = binding.Context(64, 8, 4)  # created later, smaller in every way
+    gpu, _ = run_gpu(big, ctx=ctx_big, options={"i_block": 32, "j_split": 3})
+    _full_check(oracle, big, gpu)
+    assert np.all(gpu["nbr_count"][:4] == big.state.n - 1)
+    ctx_small.close()
+    ctx_big.close()
