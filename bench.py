@@ -210,8 +210,24 @@ def run_sweep(args):
         torch.cuda.synchronize()
         us = ev[0].elapsed_time(ev[1]) / reps * 1e3
         us_fused = ev[2].elapsed_time(ev[3]) / reps * 1e3
+        # the same fused step (predictor + force + gather) captured once in a CUDA graph and replayed: the calls only
+        # enqueue kernels, so the enqueue cost of Python/ctypes and of three launches drops out
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            ctx.nb_predict_j(s.t)
+            ctx.nb_regular_force(i_idx, r_s, s.t, out=out)
+        graph.replay()
+        gv = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        gv[0].record()
+        for _ in range(reps):
+            graph.replay()
+        gv[1].record()
+        torch.cuda.synchronize()
+        us_graph = gv[0].elapsed_time(gv[1]) / reps * 1e3
+        del graph
         info = ctx.nb_last_launch_info()
-        rows.append({"n_i": n_i, "us_per_call": us, "gpairs": n_i * s.n / us / 1e3, "us_fused": us_fused,
+        rows.append({"n_i": n_i, "us_per_call": us, "gpairs": n_i * s.n / us / 1e3, "us_fused": us_fused, "us_fused_graph": us_graph,
                      "rows_per_cta": info["rows_per_cta"], "j_chunks": info["j_chunks"], "ctas": info["ctas"]})
     print(json.dumps({"metric": METRIC, "unit": UNIT, "config": {"workload": "BASELINE.json configs[2] block sweep",
                                                                  "n": s.n, "timing": "back-to-back calls between two events"},

@@ -217,3 +217,35 @@ def test_two_contexts_with_different_caps(oracle):
     assert np.all(gpu["nbr_count"][:4] == big.state.n - 1)
     ctx_small.close()
     ctx_big.close()
+
+
+def test_calls_are_cuda_graph_capturable(oracle):
+    """Device-pointer calls only enqueue kernels on the caller's stream (no allocation, no synchronisation), so a
+    whole step -- predictor, force, gather -- can be captured once and replayed (small active blocks are bound by
+    enqueue latency otherwise)."""
+    wl = _wl(oracle, 5000, 96, 20, 64)
+    s = wl.state
+    ctx = binding.Context(s.n, wl.n_i, wl.cap)
+    ctx.set_state(s)
+    dev = ctx.workspace.device
+    i_idx = torch.from_numpy(np.ascontiguousarray(wl.i_idx, dtype=np.int32)).to(dev)
+    r_s = torch.from_numpy(np.ascontiguousarray(wl.r_s)).to(dev)
+    out = ctx.alloc_outputs(wl.n_i)
+    ctx.nb_predict_j(s.t)
+    ctx.nb_regular_force(i_idx, r_s, s.t, out=out)  # warm-up outside the capture
+    torch.cuda.synchronize()
+    ref = {k: v.clone() for k, v in out.items()}
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        ctx.nb_predict_j(s.t)
+        ctx.nb_regular_force(i_idx, r_s, s.t, out=out)
+    for k in ("acc", "jerk", "nbr_count", "nbr_list"):
+        out[k].zero_()
+    graph.replay()
+    graph.replay()
+    torch.cuda.synchronize()
+    for k in ("acc", "jerk", "nbr_count", "n_overflow"):
+        assert torch.equal(out[k], ref[k]), k
+    gpu = {k: v.cpu().numpy() for k, v in out.items()}
+    _full_check(oracle, wl, gpu)
+    ctx.close()
