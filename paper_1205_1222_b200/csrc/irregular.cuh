@@ -35,12 +35,20 @@ struct PredRecord {  // one particle's share of a packed pair record
     float xh, yh, zh, m, xl, yl, zl, vx, vy, vz;
 };
 
+// Gather one particle: the five 16-byte quarters of its pair record (five vector loads, each one sector access per
+// lane), then the particle's half of each.  Scalar loads of the ten words would make twice as many scattered
+// requests, and the L1/TEX stage that serves scattered requests is what bounds this kernel (ncu: L1/TEX 82 % busy,
+// L2 51 %, issue slots 25 % with scalar loads; keeping 2-8 gathers in flight per lane changed nothing).
 __device__ __forceinline__ PredRecord load_record(const float4* packed, int32_t j) {
-    const float* rec = reinterpret_cast<const float*>(packed + (size_t)(j >> 1) * kQuadsPerPair) + (j & 1);
+    const float4* rec = packed + (size_t)(j >> 1) * kQuadsPerPair;
+    const float4 q0 = __ldg(rec), q1 = __ldg(rec + 1), q2 = __ldg(rec + 2), q3 = __ldg(rec + 3), q4 = __ldg(rec + 4);
+    const bool odd = j & 1;
     PredRecord r;
-    r.xh = __ldg(rec + 0); r.yh = __ldg(rec + 2); r.zh = __ldg(rec + 4); r.m = __ldg(rec + 6);
-    r.vx = __ldg(rec + 8); r.vy = __ldg(rec + 10); r.vz = __ldg(rec + 12);
-    r.xl = __ldg(rec + 14); r.yl = __ldg(rec + 16); r.zl = __ldg(rec + 18);
+    r.xh = odd ? q0.y : q0.x; r.yh = odd ? q0.w : q0.z;
+    r.zh = odd ? q1.y : q1.x; r.m = odd ? q1.w : q1.z;
+    r.vx = odd ? q2.y : q2.x; r.vy = odd ? q2.w : q2.z;
+    r.vz = odd ? q3.y : q3.x; r.xl = odd ? q3.w : q3.z;
+    r.yl = odd ? q4.y : q4.x; r.zl = odd ? q4.w : q4.z;
     return r;
 }
 
