@@ -310,9 +310,9 @@ def run_gpu_arm(args):
         irr_pairs = int(torch.clamp(out["nbr_count"], max=wl.cap).sum().item())
         irr = {"kernel": "irregular_kernel", "pairs": irr_pairs, "ms": t_irr * 1e3,
                "value": irr_pairs / t_irr / 1e9, "unit": UNIT, "bound": "l2-gather",
-               "gathered_gb_per_s": irr_pairs * 40 / t_irr / 1e9,
-               "note": "eq. (7), (8) over the neighbour lists of the last step; 40 B of packed record gathered per pair "
-                       "(L2-resident at this N); no measured L2 peak exists in MEASURED_PEAKS.json, so no fraction is given"}
+               "gathered_gb_per_s": irr_pairs * 48 / t_irr / 1e9,
+               "note": "eq. (7), (8) over the neighbour lists of the last step; one 48 B particle-major record gathered per pair "
+                       "(L2-resident at this N); bound by the L1/TEX sector rate for scattered accesses (profiles/), for which no measured peak exists in MEASURED_PEAKS.json, so no fraction is given"}
 
     # ---- e2e: C-ABI call with HOST (pinned) buffers, copies inside the timed region
     e2e = None
@@ -347,7 +347,7 @@ def run_gpu_arm(args):
     nsm = torch.cuda.get_device_properties(local).multi_processor_count
     peak_tf = nsm * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
     ach_tf = wl.pairs * FLOPS_PER_PAIR / t_force / 1e12
-    pred_bytes = s.n * (112 + 40)
+    pred_bytes = s.n * (112 + 40 + 48)  # state read; pair-interleaved and particle-major records written
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True,
@@ -368,9 +368,9 @@ def run_gpu_arm(args):
         "roofline_predictor": {"bound": "hbm", "kernel": "predict_kernel", "achieved": pred_bytes / t_pred / 1e9,
                                "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": pred_bytes / t_pred / 1e9 / peaks["hbm_gbs"],
                                "traffic": None, "ms": t_pred * 1e3,
-                               "note": f"152 B/j algorithmic (112 read + 40 written), peak {peaks['src']} copy bandwidth; ms is the "
+                               "note": f"200 B/j algorithmic (112 read + 40 + 48 written), peak {peaks['src']} copy bandwidth; ms is the "
                                        f"interval between two events around ONE launch inside the step and includes the "
-                                       f"event-to-kernel latency (the kernel alone: 25.0 us = 6.4 TB/s in "
+                                       f"event-to-kernel latency (the kernel alone, before the 48 B particle-major copy was added: 25.0 us in "
                                        f"profiles/r1_bench_c5_launches.md)"},
         "launch": info, "gpu_launches": int(info["launches"] + 1) * args.steps,
         "mean_neighbours": mean_cnt, "overflow_rows": n_over, "clocks": clocks, "e2e": e2e,

@@ -47,7 +47,7 @@ const char* nb_strerror(int code);
 
 /* Bytes of device workspace nb_create needs for up to n_max j-particles, active blocks of up to n_i_max rows
  * and neighbour lists of nbr_cap entries per row (1 <= nbr_cap <= 8192).  Holds the packed predicted j-records
- * (40 B per j) and, for the row blocks whose j-range is split over several CTAs, 56 B of
+ * (40 B per j, pair-interleaved, plus a 48 B particle-major copy for nb_irregular_force) and, for the row blocks whose j-range is split over several CTAs, 56 B of
  * partial sums per (row, j-chunk): at most 112 MB, plus 4 B per row of list-slot counters.  nb_create clears the
  * counters once; every call leaves them cleared.  Returns 0 if an argument is invalid. */
 size_t nb_workspace_bytes(int64_t n_max, int64_t n_i_max, int32_t nbr_cap);

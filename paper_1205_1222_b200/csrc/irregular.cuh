@@ -5,7 +5,7 @@
 // to be gathered "from non-contiguous addresses indicated by the neighbour list".
 //
 // Here: one WARP per row.  The lanes stride over the row's list (coalesced index loads), each lane gathers its j
-// from the packed predicted records (nbreg_common.cuh) -- which at N <= 2^20 stay resident in the 126 MB L2 --
+// from the particle-major predicted records (nbreg_common.cuh) -- which at N <= 2^20 stay resident in the 126 MB L2 --
 // and evaluates the pair in fp32 on "two-float" coordinate differences, always with the low words (PAPER.md:138:
 // "full single precision ... may not be accurate enough during close encounters. Thus, we employ the so-called
 // 'two-float' technique").  A lane holds at most cap/32 terms in fp32 ("single precision turned out to be
@@ -18,7 +18,7 @@
 namespace nbreg {
 
 struct IrregularArgs {
-    const float4* packed;      // packed predicted j-records
+    const float4* gather;      // particle-major predicted records, 3 float4 per particle (nbreg_common.cuh)
     int32_t n;                 // j-particles (entries outside [0, n) are ignored)
     int32_t n_i;
     int32_t list_stride;       // ints per row of nbr_list
@@ -35,20 +35,17 @@ struct PredRecord {  // one particle's share of a packed pair record
     float xh, yh, zh, m, xl, yl, zl, vx, vy, vz;
 };
 
-// Gather one particle: the five 16-byte quarters of its pair record (five vector loads, each one sector access per
-// lane), then the particle's half of each.  Scalar loads of the ten words would make twice as many scattered
-// requests, and the L1/TEX stage that serves scattered requests is what bounds this kernel (ncu: L1/TEX 82 % busy,
-// L2 51 %, issue slots 25 % with scalar loads; keeping 2-8 gathers in flight per lane changed nothing).
-__device__ __forceinline__ PredRecord load_record(const float4* packed, int32_t j) {
-    const float4* rec = packed + (size_t)(j >> 1) * kQuadsPerPair;
-    const float4 q0 = __ldg(rec), q1 = __ldg(rec + 1), q2 = __ldg(rec + 2), q3 = __ldg(rec + 3), q4 = __ldg(rec + 4);
-    const bool odd = j & 1;
+// Gather one particle: three 16-byte loads from its 48-byte particle-major record (two sectors).  This kernel sits on
+// the L1/TEX sector rate for scattered accesses (profiles/r1_irregular_kernel_ncu_full.md), so what counts is
+// the number of sector accesses per gathered particle: 3 here, 5 from the pair-interleaved records of the
+// regular-force kernel, 10 with scalar loads.
+__device__ __forceinline__ PredRecord load_record(const float4* gather, int32_t j) {
+    const float4* rec = gather + (size_t)j * kGatherQuads;
+    const float4 g0 = __ldg(rec), g1 = __ldg(rec + 1), g2 = __ldg(rec + 2);
     PredRecord r;
-    r.xh = odd ? q0.y : q0.x; r.yh = odd ? q0.w : q0.z;
-    r.zh = odd ? q1.y : q1.x; r.m = odd ? q1.w : q1.z;
-    r.vx = odd ? q2.y : q2.x; r.vy = odd ? q2.w : q2.z;
-    r.vz = odd ? q3.y : q3.x; r.xl = odd ? q3.w : q3.z;
-    r.yl = odd ? q4.y : q4.x; r.zl = odd ? q4.w : q4.z;
+    r.xh = g0.x; r.yh = g0.y; r.zh = g0.z; r.m = g0.w;
+    r.xl = g1.x; r.yl = g1.y; r.zl = g1.z; r.vx = g1.w;
+    r.vy = g2.x; r.vz = g2.y;
     return r;
 }
 
@@ -57,7 +54,7 @@ __global__ void __launch_bounds__(kIrrWarps * 32) irregular_kernel(IrregularArgs
     const int64_t row = (int64_t)blockIdx.x * kIrrWarps + (threadIdx.x >> 5);
     if (row >= a.n_i) return;  // warp-uniform
     const int32_t i = a.i_idx[row];
-    const PredRecord pi = load_record(a.packed, i);
+    const PredRecord pi = load_record(a.gather, i);
     const int32_t len = min(a.nbr_count[row], a.list_stride);
     const int32_t* list = a.nbr_list + (size_t)row * a.list_stride;
 
@@ -65,7 +62,7 @@ __global__ void __launch_bounds__(kIrrWarps * 32) irregular_kernel(IrregularArgs
     for (int32_t e = lane; e < len; e += 32) {
         const int32_t j = list[e];
         if (j == i || j < 0 || j >= a.n) continue;
-        const PredRecord pj = load_record(a.packed, j);
+        const PredRecord pj = load_record(a.gather, j);
         // two-float differences: (xh_j - xh_i) + (xl_j - xl_i)
         const float dx = (pj.xh - pi.xh) + (pj.xl - pi.xl);
         const float dy = (pj.yh - pi.yh) + (pj.yl - pi.yl);

@@ -62,6 +62,7 @@ struct Plan {
 struct WorkspaceLayout {
     size_t packed_off, packed_bytes;
     size_t psum_off, psum_bytes;
+    size_t gather_off, gather_bytes;  // particle-major predicted records, 48 B per j
     size_t vmax_off, vmax_bytes;   // float speed bound per 256 consecutive j (predictor -> velocity criterion)
     size_t slot_off, slot_bytes;   // int32 list-slot counters of the j-split rows (zero between calls)
     size_t ctl_off, ctl_bytes;     // int32 {overflow count, gather ticket} (zero between calls)
@@ -88,6 +89,7 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
     };
     place((size_t)n_pad * kBytesPerJ, w.packed_off, w.packed_bytes);
     place((size_t)w.row_chunk_limit * 7 * sizeof(double), w.psum_off, w.psum_bytes);  // acc, jerk, pot
+    place((size_t)n_pad * kGatherQuads * sizeof(float4), w.gather_off, w.gather_bytes);
     place((size_t)(n_pad / kJPad) * sizeof(float), w.vmax_off, w.vmax_bytes);
     place((size_t)(n_i_max + 512) * sizeof(int32_t), w.slot_off, w.slot_bytes);
     place(64, w.ctl_off, w.ctl_bytes);
@@ -283,6 +285,7 @@ int run_predict(nb_ctx* c, double t, cudaStream_t st, double* xp_out, double* vp
     pa.x0 = c->x0; pa.v0 = c->v0; pa.a0 = c->a0; pa.j0 = c->j0; pa.m = c->m; pa.t0 = c->t0;
     pa.t = t;
     pa.packed = reinterpret_cast<float4*>(c->ws + c->lay.packed_off);
+    pa.gather = reinterpret_cast<float4*>(c->ws + c->lay.gather_off);
     pa.tile_vmax = reinterpret_cast<float*>(c->ws + c->lay.vmax_off);
     pa.xp_out = xp_out;
     pa.vp_out = vp_out;
@@ -527,7 +530,7 @@ int nb_irregular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const int32
     }
     if (n_i == 0) return NB_OK;
     IrregularArgs ia{};
-    ia.packed = reinterpret_cast<const float4*>(c->ws + c->lay.packed_off);
+    ia.gather = reinterpret_cast<const float4*>(c->ws + c->lay.gather_off);
     ia.n = (int32_t)c->n;
     ia.n_i = n_i;
     ia.list_stride = list_stride;

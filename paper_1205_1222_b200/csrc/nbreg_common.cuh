@@ -10,7 +10,10 @@
 //     q3 = { vz0, vz1, xl0, xl1 }     position low words    (xl = fl32(x_p - xh): "two-float")
 //     q4 = { yl0, yl1, zl0, zl1 }
 // The low words sit at the end of the record: the common (far-pair) path of the force kernel never loads them.
-// = 40 B per j.  The array is padded with massless dummies parked far away up to a multiple of kJPad.
+// = 40 B per j.  A second, PARTICLE-major copy serves kernels that gather single particles by index (the irregular
+// force, irregular.cuh): three float4 per particle, { xh, yh, zh, m } { xl, yl, zl, vx } { vy, vz, 0, 0 } = 48 B in
+// two 32-byte sectors, against three or four sectors and five accesses for a particle's half of a pair record.
+// The pair array is padded with massless dummies parked far away up to a multiple of kJPad.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -18,6 +21,7 @@
 namespace nbreg {
 
 constexpr int kQuadsPerPair = 5;       // float4 per packed j-pair
+constexpr int kGatherQuads = 3;        // float4 per particle of the particle-major copy (below)
 constexpr int kBytesPerJ = 40;         // packed bytes per j-particle
 constexpr int kJPad = 256;             // packed array length is a multiple of this (largest j-tile)
 constexpr float kFarAway = 1.0e18f;    // coordinate of the massless padding particles

@@ -19,6 +19,7 @@ struct PredictArgs {
     const double* t0;
     double t;
     float4* packed;
+    float4* gather;    // [n][3] particle-major copy of the predicted records (nbreg_common.cuh)
     float* tile_vmax;  // [n_pad / 256] upper bound of |v_p| over each block of 256 consecutive particles
     double* xp_out;  // fp64 outputs (test hook), used only when WRITE_F64
     double* vp_out;
@@ -116,6 +117,17 @@ __global__ void __launch_bounds__(256) predict_kernel(PredictArgs a) {
         o[2] = make_float4(vf[0], vf[3], vf[1], vf[4]);
         o[3] = make_float4(vf[2], vf[5], xl[0], xl[3]);
         o[4] = make_float4(xl[1], xl[4], xl[2], xl[5]);
+        if (j0 < a.n) {  // particle-major copy: the pair's two records are contiguous (96 B)
+            float4* g = a.gather + kGatherQuads * j0;
+            g[0] = make_float4(xh[0], xh[1], xh[2], mf[0]);
+            g[1] = make_float4(xl[0], xl[1], xl[2], vf[0]);
+            g[2] = make_float4(vf[1], vf[2], 0.f, 0.f);
+            if (j0 + 1 < a.n) {
+                g[3] = make_float4(xh[3], xh[4], xh[5], mf[1]);
+                g[4] = make_float4(xl[3], xl[4], xl[5], vf[3]);
+                g[5] = make_float4(vf[4], vf[5], 0.f, 0.f);
+            }
+        }
     }
 }
 
