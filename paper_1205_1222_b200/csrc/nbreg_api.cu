@@ -17,10 +17,16 @@
 
 using namespace nbreg;
 
-// Resident 256-thread CTAs per SM the one-i-per-thread force kernels are compiled for (register cap
-// 65536 / (256 * NBREG_CTAS256)); smaller CTA shapes scale it so that the warps per SM stay the same.
+// Resident 256-thread CTAs per SM the 256-row force kernel is compiled for (register cap 65536 / (256 *
+// NBREG_CTAS256)).
 #ifndef NBREG_CTAS256
 #define NBREG_CTAS256 3
+#endif
+// Resident warps per SM the smaller shapes (128, 64, 32 rows per CTA) are compiled for: 28 = 65536 / (72 * 32), a
+// granularity the 256-thread shape cannot reach (3 CTAs = 24 warps, 4 would need <= 64 registers).  Measured on
+// B200: 28 warps are 1-3 % faster than 24-26 (config 5: 1064 against 1054 Gpairs/s).
+#ifndef NBREG_WARPS_SMALL
+#define NBREG_WARPS_SMALL 28
 #endif
 
 namespace {
@@ -214,8 +220,9 @@ Plan make_plan(const Machine* c, int32_t n_i, int64_t opt_i_block, int64_t opt_j
             if (kShapes[k].rows == opt_i_block) shape = k;
         return plan_for_shape(c, n_i, shape, opt_j_split);
     }
-    // smaller CTAs pay a little more for staging the j-tiles (fewer warps share one bulk copy)
-    const double penalty[4] = {1.0, 1.02, 1.04, 1.06};
+    // measured preferences: the 128-row shape holds 28 warps per SM against 24 of the 256-row shape (1-3 % faster);
+    // still smaller CTAs pay a little more for staging the j-tiles (fewer warps share one bulk copy)
+    const double penalty[4] = {1.02, 1.0, 1.02, 1.04};
     Plan best{};
     double best_cost = 1e300;
     for (int k = 0; k < 4; ++k) {
@@ -261,9 +268,9 @@ int force_dispatch_v(int shape, int* per_sm, const Plan* p, const ForceArgs* fa,
             : launch_force<IPT, WARPS, JT, MINB, VEL, POT>(*p, *fa, st))
     switch (shape) {
         case 0: return NB_SHAPE(1, 8, 256, NBREG_CTAS256);
-        case 1: return NB_SHAPE(1, 4, 128, 2 * NBREG_CTAS256);
-        case 2: return NB_SHAPE(1, 2, 128, 4 * NBREG_CTAS256);
-        case 3: return NB_SHAPE(1, 1, 64, 8 * NBREG_CTAS256);
+        case 1: return NB_SHAPE(1, 4, 128, NBREG_WARPS_SMALL / 4);
+        case 2: return NB_SHAPE(1, 2, 128, NBREG_WARPS_SMALL / 2);
+        case 3: return NB_SHAPE(1, 1, 64, NBREG_WARPS_SMALL);
         default: return NB_SHAPE(2, 8, 256, 1);
     }
 #undef NB_SHAPE
