@@ -49,7 +49,7 @@ constexpr int kNumShapes = 5;
 struct Shape {
     int rows, ipt, warps, jt;
 };
-constexpr Shape kShapes[kNumShapes] = {{256, 1, 8, 256}, {128, 1, 4, 128}, {64, 1, 2, 128}, {32, 1, 1, 64},
+constexpr Shape kShapes[kNumShapes] = {{256, 1, 8, 256}, {128, 1, 4, 256}, {64, 1, 2, 128}, {32, 1, 1, 64},
                                        {512, 2, 8, 256}};
 
 // Launch plan of the force kernel: CTA shape, how many row blocks run the whole j-range in one CTA ("main"),
@@ -268,7 +268,7 @@ int force_dispatch_v(int shape, int* per_sm, const Plan* p, const ForceArgs* fa,
             : launch_force<IPT, WARPS, JT, MINB, VEL, POT>(*p, *fa, st))
     switch (shape) {
         case 0: return NB_SHAPE(1, 8, 256, NBREG_CTAS256);
-        case 1: return NB_SHAPE(1, 4, 128, NBREG_WARPS_SMALL / 4);
+        case 1: return NB_SHAPE(1, 4, 256, NBREG_WARPS_SMALL / 4);
         case 2: return NB_SHAPE(1, 2, 128, NBREG_WARPS_SMALL / 2);
         case 3: return NB_SHAPE(1, 1, 64, NBREG_WARPS_SMALL);
         default: return NB_SHAPE(2, 8, 256, 1);
