@@ -43,8 +43,9 @@ int cuda_fail(cudaError_t e, const char* what) {
         if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
     } while (0)
 
-// CTA shapes of the force kernel.  All one-i-per-thread shapes keep the same number of resident warps per SM
-// (8 * NBREG_CTAS256); the 512-row shape (two i per thread) is only used when asked for.
+// CTA shapes of the force kernel: rows per CTA, i per thread, warps, particles per shared-memory j-tile.  The 256-row
+// shape holds NBREG_CTAS256 CTAs (24 warps) per SM, the smaller ones NBREG_WARPS_SMALL warps; the 512-row shape (two
+// i per thread) is only used when asked for ("i_block" option).
 constexpr int kNumShapes = 5;
 struct Shape {
     int rows, ipt, warps, jt;
