@@ -106,6 +106,11 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
 
 }  // namespace
 
+// nb_regular_force_host splits large active blocks into up to kHostChunks row chunks so that the device-to-host copy
+// of one chunk's outputs (the list array dominates) runs while the next chunk is computed
+constexpr int kHostChunks = 8;
+constexpr int64_t kHostChunkMinRows = 16384;
+
 struct nb_ctx {
     int device = 0;
     int num_sms = 0;
@@ -125,7 +130,9 @@ struct nb_ctx {
     // last launch
     int64_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     // host path: device mirrors owned by the context
-    cudaStream_t hstream = nullptr;
+    cudaStream_t hstream = nullptr, hcopy = nullptr;  // compute and device-to-host copy streams
+    cudaEvent_t hdone[kHostChunks] = {};              // "rows of chunk k are final"
+    int32_t* hovf = nullptr;                          // pinned: overflow count of each chunk
     unsigned char* hbuf = nullptr;
     size_t hbuf_bytes = 0;
 };
@@ -404,6 +411,13 @@ int nb_destroy(nb_ctx* c) {
         cudaStreamSynchronize(c->hstream);
         cudaStreamDestroy(c->hstream);
     }
+    if (c->hcopy) {
+        cudaStreamSynchronize(c->hcopy);
+        cudaStreamDestroy(c->hcopy);
+    }
+    for (int k = 0; k < kHostChunks; ++k)
+        if (c->hdone[k]) cudaEventDestroy(c->hdone[k]);
+    if (c->hovf) cudaFreeHost(c->hovf);
     if (c->hbuf) cudaFree(c->hbuf);
     if (c->ws_owned && c->ws) cudaFree(c->ws);
     delete c;
@@ -559,6 +573,10 @@ int nb_regular_force_host(nb_ctx* c, int64_t n, const double* x0, const double* 
     if (n_i > 0 && (!i_idx || !r_s || !acc || !jerk || !nbr_count || !nbr_list)) return NB_E_INVAL;
     NB_CUDA(cudaSetDevice(c->device));
     if (!c->hstream) NB_CUDA(cudaStreamCreateWithFlags(&c->hstream, cudaStreamNonBlocking));
+    if (!c->hcopy) NB_CUDA(cudaStreamCreateWithFlags(&c->hcopy, cudaStreamNonBlocking));
+    for (int k = 0; k < kHostChunks; ++k)
+        if (!c->hdone[k]) NB_CUDA(cudaEventCreateWithFlags(&c->hdone[k], cudaEventDisableTiming));
+    if (!c->hovf) NB_CUDA(cudaMallocHost(&c->hovf, kHostChunks * sizeof(int32_t)));
     // device mirrors, carved from one allocation sized for n_max / n_i_max / cap
     const size_t nmax = (size_t)c->n_max, imax = (size_t)c->n_i_max;
     size_t off = 0;
@@ -576,8 +594,8 @@ int nb_regular_force_host(nb_ctx* c, int64_t n, const double* x0, const double* 
         c->hbuf_bytes = off;
     }
     unsigned char* b = c->hbuf;
-    cudaStream_t st = c->hstream;
-    const size_t nn = (size_t)n, ni = (size_t)n_i;
+    cudaStream_t st = c->hstream, cs = c->hcopy;
+    const size_t nn = (size_t)n, ni = (size_t)n_i, cap = (size_t)c->cap;
     NB_CUDA(cudaMemcpyAsync(b + o_x0, x0, nn * 24, cudaMemcpyHostToDevice, st));
     NB_CUDA(cudaMemcpyAsync(b + o_v0, v0, nn * 24, cudaMemcpyHostToDevice, st));
     NB_CUDA(cudaMemcpyAsync(b + o_a0, a0, nn * 24, cudaMemcpyHostToDevice, st));
@@ -591,18 +609,38 @@ int nb_regular_force_host(nb_ctx* c, int64_t n, const double* x0, const double* 
     int rc = nb_set_j(c, n, (const double*)(b + o_x0), (const double*)(b + o_v0), (const double*)(b + o_a0),
                       (const double*)(b + o_j0), (const double*)(b + o_m), (const double*)(b + o_t0));
     if (rc != NB_OK) return rc;
-    rc = nb_regular_force(c, n_i, (const int32_t*)(b + o_idx), (const double*)(b + o_rs), t, (double*)(b + o_acc),
-                          (double*)(b + o_jrk), (int32_t*)(b + o_cnt), (int32_t*)(b + o_lst), (int32_t*)(b + o_ovf),
-                          st);
-    if (rc != NB_OK) return rc;
-    if (n_i > 0) {
-        NB_CUDA(cudaMemcpyAsync(acc, b + o_acc, ni * 24, cudaMemcpyDeviceToHost, st));
-        NB_CUDA(cudaMemcpyAsync(jerk, b + o_jrk, ni * 24, cudaMemcpyDeviceToHost, st));
-        NB_CUDA(cudaMemcpyAsync(nbr_count, b + o_cnt, ni * 4, cudaMemcpyDeviceToHost, st));
-        NB_CUDA(cudaMemcpyAsync(nbr_list, b + o_lst, ni * (size_t)c->cap * 4, cudaMemcpyDeviceToHost, st));
+    // row chunks: compute chunk k on the compute stream, copy its rows back on the copy stream meanwhile
+    // ... when that pays: a row costs ~N ns of compute per 1000 j and (4 cap + 52) B of copy at ~50 GB/s; splitting a
+    // block costs a few per cent of kernel efficiency, so it is done only if the copy is >= 10 % of the compute
+    const bool overlap_pays = (double)(4 * (int64_t)c->cap + 52) / 50.0 >= 0.1 * (double)n / 1000.0;
+    int64_t rows_per_chunk = std::max<int64_t>(kHostChunkMinRows, (n_i + kHostChunks - 1) / kHostChunks);
+    rows_per_chunk = round_up(rows_per_chunk, 1024);
+    if (!overlap_pays) rows_per_chunk = round_up(std::max<int64_t>(n_i, 1), 1024);
+    const int n_chunks = n_i > 0 ? (int)((n_i + rows_per_chunk - 1) / rows_per_chunk) : 1;
+    for (int k = 0; k < n_chunks; ++k) {
+        const size_t r0 = (size_t)k * (size_t)rows_per_chunk;
+        const size_t nr = n_i > 0 ? std::min<size_t>((size_t)rows_per_chunk, ni - r0) : 0;
+        int32_t* d_ovf = (int32_t*)(b + o_ovf) + k;
+        rc = nb_regular_force(c, (int32_t)nr, (const int32_t*)(b + o_idx) + r0, (const double*)(b + o_rs) + r0, t,
+                              (double*)(b + o_acc) + 3 * r0, (double*)(b + o_jrk) + 3 * r0, (int32_t*)(b + o_cnt) + r0,
+                              (int32_t*)(b + o_lst) + r0 * cap, d_ovf, st);
+        if (rc != NB_OK) return rc;
+        NB_CUDA(cudaEventRecord(c->hdone[k], st));
+        NB_CUDA(cudaStreamWaitEvent(cs, c->hdone[k], 0));
+        if (nr > 0) {
+            NB_CUDA(cudaMemcpyAsync(acc + 3 * r0, (double*)(b + o_acc) + 3 * r0, nr * 24, cudaMemcpyDeviceToHost, cs));
+            NB_CUDA(cudaMemcpyAsync(jerk + 3 * r0, (double*)(b + o_jrk) + 3 * r0, nr * 24, cudaMemcpyDeviceToHost, cs));
+            NB_CUDA(cudaMemcpyAsync(nbr_count + r0, (int32_t*)(b + o_cnt) + r0, nr * 4, cudaMemcpyDeviceToHost, cs));
+            NB_CUDA(cudaMemcpyAsync(nbr_list + r0 * cap, (int32_t*)(b + o_lst) + r0 * cap, nr * cap * 4,
+                                    cudaMemcpyDeviceToHost, cs));
+        }
+        NB_CUDA(cudaMemcpyAsync(c->hovf + k, d_ovf, sizeof(int32_t), cudaMemcpyDeviceToHost, cs));
     }
-    NB_CUDA(cudaMemcpyAsync(n_overflow, b + o_ovf, 4, cudaMemcpyDeviceToHost, st));
     NB_CUDA(cudaStreamSynchronize(st));
+    NB_CUDA(cudaStreamSynchronize(cs));
+    int32_t total_overflow = 0;
+    for (int k = 0; k < n_chunks; ++k) total_overflow += c->hovf[k];
+    *n_overflow = total_overflow;
     // the registered pointers are the context's own mirrors; they stay valid, but a new host call overwrites them
     return NB_OK;
 }

@@ -249,3 +249,32 @@ def test_calls_are_cuda_graph_capturable(oracle):
     gpu = {k: v.cpu().numpy() for k, v in out.items()}
     _full_check(oracle, wl, gpu)
     ctx.close()
+
+
+def test_host_entry_point_in_row_chunks(oracle):
+    """nb_regular_force_host splits blocks of more than 16384 rows into row chunks (copy-back overlapped with the
+    next chunk): same lists and counts as the device entry point, sums equal to rounding, overflow count summed."""
+    wl = _wl(oracle, 2500, 40001, 20, 32)
+    wl.r_s[::1000] *= 3.0  # a few overflowing rows in every chunk
+    dev_out, _ = run_gpu(wl)
+    s = wl.state
+    ctx = binding.Context(s.n, wl.n_i, wl.cap)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    out = dict(acc=torch.empty((wl.n_i, 3), dtype=torch.float64).pin_memory(),
+               jerk=torch.empty((wl.n_i, 3), dtype=torch.float64).pin_memory(),
+               nbr_count=torch.empty(wl.n_i, dtype=torch.int32).pin_memory(),
+               nbr_list=torch.full((wl.n_i, wl.cap), -7, dtype=torch.int32).pin_memory(),
+               n_overflow=torch.zeros(1, dtype=torch.int32).pin_memory())
+    ctx.nb_regular_force_host(pin(s.x0), pin(s.v0), pin(s.a0), pin(s.j0), pin(s.m), pin(s.t0),
+                              pin(wl.i_idx.astype(np.int32)), pin(wl.r_s), s.t, out)
+    host = {k: v.numpy() for k, v in out.items()}
+    assert np.array_equal(host["nbr_count"], dev_out["nbr_count"])
+    assert int(host["n_overflow"][0]) == int(dev_out["n_overflow"][0]) >= 40
+    ok = dev_out["nbr_count"] <= wl.cap
+    for q in np.nonzero(ok)[0][::7]:
+        c = dev_out["nbr_count"][q]
+        assert np.array_equal(host["nbr_list"][q, :c], dev_out["nbr_list"][q, :c])
+    assert parity.relerr(host["acc"], dev_out["acc"]).max() < 5e-7
+    assert parity.relerr(host["jerk"], dev_out["jerk"]).max() < 5e-6
+    _full_check(oracle, wl, host)
+    ctx.close()
