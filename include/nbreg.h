@@ -48,7 +48,7 @@ const char* nb_strerror(int code);
 /* Bytes of device workspace nb_create needs for up to n_max j-particles, active blocks of up to n_i_max rows
  * and neighbour lists of nbr_cap entries per row (1 <= nbr_cap <= 8192).  Holds the packed predicted j-records
  * (40 B per j, pair-interleaved, plus a 48 B particle-major copy for nb_irregular_force) and, for the row blocks whose j-range is split over several CTAs, 56 B of
- * partial sums per (row, j-chunk): at most 112 MB, plus 4 B per row of list-slot counters.  nb_create clears the
+ * partial sums per (row, j-chunk): at most 112 MB, plus ~24 B per row for list-slot counters and the row ordering.  nb_create clears the
  * counters once; every call leaves them cleared.  Returns 0 if an argument is invalid. */
 size_t nb_workspace_bytes(int64_t n_max, int64_t n_i_max, int32_t nbr_cap);
 
@@ -143,6 +143,8 @@ int nb_regular_force_host(nb_ctx* ctx, int64_t n, const double* x0, const double
 /* Tuning knobs (tests and benchmarks).  key:
  *   "j_split"   force the number of j-chunks per row for ALL row blocks (0 = automatic; 1 = never split)
  *   "i_block"   force the rows per CTA: 32, 64, 128, 256 or 512 (0 = automatic)
+ *   "order_rows" 1 (default): large enough blocks are processed in Morton order of the predicted positions
+ *               (results go to the caller's rows all the same); 0: always in the order given; 2: always ordered
  * Returns NB_E_INVAL for an unknown key or value. */
 int nb_set_option(nb_ctx* ctx, const char* key, int64_t value);
 

@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "nbreg_api.cu")
 DEPS = [os.path.join(HERE, "csrc", f) for f in
-        ("nbreg_api.cu", "nbreg_common.cuh", "predict.cuh", "force.cuh", "gather.cuh", "irregular.cuh")] + \
+        ("nbreg_api.cu", "nbreg_common.cuh", "predict.cuh", "force.cuh", "gather.cuh", "irregular.cuh", "order.cuh")] + \
        [os.path.join(os.path.dirname(HERE), "include", "nbreg.h")]
 LIB = os.environ.get("NBREG_LIB") or os.path.join(HERE, "libnbreg.so")  # NBREG_LIB: use a library built elsewhere
 

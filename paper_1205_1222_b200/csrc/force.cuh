@@ -49,6 +49,9 @@ struct ForceArgs {
     int32_t cap;
     const int32_t* i_idx;
     const double* r_s;
+    // Rows are processed in the order perm gives (Morton order of the predicted positions, order.cuh; null = as
+    // given): thread "row" below is the LOGICAL row, perm[row] the caller's row all inputs and outputs refer to.
+    const int32_t* perm;
     const double* dtr;       // VEL: regular time-step per row, eq. (3)
     const float* tile_vmax;  // VEL: speed bound per 256 consecutive j (predict.cuh)
     double* pot;             // POT: sum m_j / r over the summed pairs ("fo.pot += mrinv1")
@@ -297,7 +300,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         const int64_t row = (int64_t)row_block * kRows + u * kThreads + tid;
         rows[u] = row;
         const bool live = row < a.n_i;
-        const int32_t i = live ? a.i_idx[row] : 0;
+        const int64_t orow = (live && a.perm) ? a.perm[row] : row;  // the caller's row
+        const int32_t i = live ? a.i_idx[orow] : 0;
         const float* rec = reinterpret_cast<const float*>(a.packed + (size_t)(i >> 1) * kQuadsPerPair);
         const int h = i & 1;
         const float xh = rec[0 + h], yh = rec[2 + h], zh = rec[4 + h];
@@ -306,7 +310,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         I[u].nxh = -xh; I[u].nyh = -yh; I[u].nzh = -zh;
         I[u].nxl = -xl; I[u].nyl = -yl; I[u].nzl = -zl;
         I[u].nvx = -vx; I[u].nvy = -vy; I[u].nvz = -vz;
-        const double rs = live ? a.r_s[row] : 0.0;
+        const double rs = live ? a.r_s[orow] : 0.0;
         const float h2 = __double2float_rn(rs * rs);
         // dead rows (past n_i) get h2 < 0: nothing is ever a neighbour, nothing is written
         I[u].h2 = live ? fmaxf(h2, 1.17549435e-38f) : -1.f;
@@ -314,9 +318,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         const float xmax = fmaxf(fabsf(xh), fmaxf(fabsf(yh), fabsf(zh)));
         I[u].hfar2 = live ? fmaxf(I[u].h2 * 1.0009765625f, kFarFraction2 * xmax * xmax) : -1.f;
         if (VEL) {
-            const float dtr = live ? fabsf(__double2float_rn(a.dtr[row])) : 0.f;
+            const float dtr = live ? fabsf(__double2float_rn(a.dtr[orow])) : 0.f;
             const float vi = sqrtf(vx * vx + vy * vy + vz * vz) * 1.000001f;
-            I[u].dtr = live ? __double2float_rn(a.dtr[row]) : 0.f;
+            I[u].dtr = live ? __double2float_rn(a.dtr[orow]) : 0.f;
             I[u].hfar_x = live ? sqrtf(kFarFraction2) * xmax : 0.f;  // dead rows: hfar2 = 0, never near
             I[u].hfar_r = live ? fmaf(dtr, vi, sqrtf(I[u].h2) * 1.00048828125f) : 0.f;
         }
@@ -325,7 +329,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         I[u].cnt = 0;
         I[u].pend_j = -1;
         I[u].pend_pos = 0;
-        I[u].list = a.nbr_list + (size_t)row * a.cap;
+        I[u].list = a.nbr_list + (size_t)orow * a.cap;
         accum_zero(s[u]);
 #pragma unroll
         for (int c = 0; c < kSums; ++c) sum[u][c] = 0.0;
@@ -403,15 +407,16 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
         const int64_t row = rows[u];
+        const int64_t orow = (row < a.n_i && a.perm) ? a.perm[row] : row;
         if (row >= a.n_i) continue;
         if (!split) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                a.acc[row * 3 + c] = sum[u][c];
-                a.jerk[row * 3 + c] = sum[u][3 + c];
+                a.acc[orow * 3 + c] = sum[u][c];
+                a.jerk[orow * 3 + c] = sum[u][3 + c];
             }
-            if (POT) a.pot[row] = sum[u][kSums - 1];
-            a.nbr_count[row] = I[u].cnt;
+            if (POT) a.pot[orow] = sum[u][kSums - 1];
+            a.nbr_count[orow] = I[u].cnt;
             if (I[u].cnt > a.cap) atomicAdd(a.overflow_ws, 1);
         } else {
             flush_pending(I[u], a.cap);

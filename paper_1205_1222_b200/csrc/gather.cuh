@@ -19,6 +19,7 @@ namespace nbreg {
 struct GatherArgs {
     int32_t row0;              // first j-split row (rows below were written directly by the force kernel)
     int32_t n_i;
+    const int32_t* perm;       // logical row -> caller's row (null: identity), as in ForceArgs
     int32_t n_chunks;
     int32_t chunk_j;           // j-particles per chunk (tiles_per_chunk * j-tile)
     int32_t cap;
@@ -44,6 +45,7 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
     const int64_t prow = (int64_t)blockIdx.x * kGatherWarps + warp;  // row among the split rows
     const int64_t row = a.row0 + prow;
     if (row < a.n_i) {  // warp-uniform
+    const int64_t orow = a.perm ? a.perm[row] : row;
     const int S = a.n_chunks;
     const size_t rbase = (size_t)prow * S;
 
@@ -61,21 +63,21 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
 #pragma unroll
         for (int k = 0; k < 7; ++k) s[k] += __shfl_xor_sync(0xffffffffu, s[k], off);
     }
-    if (lane == 0 && a.pot) a.pot[row] = s[6];
+    if (lane == 0 && a.pot) a.pot[orow] = s[6];
     if (lane < 3) {
-        a.acc[row * 3 + lane] = (lane == 0) ? s[0] : (lane == 1) ? s[1] : s[2];
-        a.jerk[row * 3 + lane] = (lane == 0) ? s[3] : (lane == 1) ? s[4] : s[5];
+        a.acc[orow * 3 + lane] = (lane == 0) ? s[0] : (lane == 1) ? s[1] : s[2];
+        a.jerk[orow * 3 + lane] = (lane == 0) ? s[3] : (lane == 1) ? s[4] : s[5];
     }
 
     // ---- list: stable counting sort of the stored entries by chunk number
     const int32_t cnt = a.slot_count[prow];  // true count, may exceed cap
     __syncwarp();
     if (lane == 0) {
-        a.nbr_count[row] = cnt;
+        a.nbr_count[orow] = cnt;
         a.slot_count[prow] = 0;
     }
     const int32_t stored = min(cnt, a.cap);
-    int32_t* out = a.nbr_list + (size_t)row * a.cap;
+    int32_t* out = a.nbr_list + (size_t)orow * a.cap;
     int32_t* stage = stage_all + (size_t)warp * (a.cap + S);
     int32_t* bin = stage + a.cap;
     const uint32_t lt_mask = (1u << lane) - 1u;
@@ -144,7 +146,8 @@ __global__ void __launch_bounds__(kWideThreads) reduce_gather_wide_kernel(Gather
     __shared__ double warp_sum[kWideThreads / 32][7];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t prow = blockIdx.x;
-    const int64_t row = a.row0 + prow;  // grid = split rows exactly
+    const int64_t lrow = a.row0 + prow;  // grid = split rows exactly
+    const int64_t row = a.perm ? a.perm[lrow] : lrow;  // the caller's row
     const int S = a.n_chunks;
     const size_t rbase = (size_t)prow * S;
 

@@ -7,11 +7,14 @@
 #include <cmath>
 #include <cstring>
 #include <utility>
+
+#include <cub/device/device_radix_sort.cuh>
 #include <new>
 
 #include "force.cuh"
 #include "gather.cuh"
 #include "irregular.cuh"
+#include "order.cuh"
 #include "nbreg_common.cuh"
 #include "predict.cuh"
 
@@ -71,8 +74,10 @@ struct WorkspaceLayout {
     size_t psum_off, psum_bytes;
     size_t gather_off, gather_bytes;  // particle-major predicted records, 48 B per j
     size_t vmax_off, vmax_bytes;   // float speed bound per 256 consecutive j (predictor -> velocity criterion)
+    size_t sort_off, sort_bytes;   // row ordering: keys and rows, two buffers each, + the library sort's scratch
+    size_t sort_temp_bytes;
     size_t slot_off, slot_bytes;   // int32 list-slot counters of the j-split rows (zero between calls)
-    size_t ctl_off, ctl_bytes;     // int32 {overflow count, gather ticket} (zero between calls)
+    size_t ctl_off, ctl_bytes;     // int32 {overflow count, gather ticket, order ticket, -, 6 box words} (zero between calls)
     int64_t row_chunk_limit;  // (row, j-chunk) slots of partial sums
     size_t total;
 };
@@ -98,6 +103,15 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
     place((size_t)w.row_chunk_limit * 7 * sizeof(double), w.psum_off, w.psum_bytes);  // acc, jerk, pot
     place((size_t)n_pad * kGatherQuads * sizeof(float4), w.gather_off, w.gather_bytes);
     place((size_t)(n_pad / kJPad) * sizeof(float), w.vmax_off, w.vmax_bytes);
+    {
+        const int64_t ni = std::max<int64_t>(n_i_max, 1);
+        size_t temp = 0;
+        cub::DoubleBuffer<uint32_t> dk(nullptr, nullptr);
+        cub::DoubleBuffer<int32_t> dv(nullptr, nullptr);
+        cub::DeviceRadixSort::SortPairs(nullptr, temp, dk, dv, (int)ni, 0, 30);
+        w.sort_temp_bytes = (size_t)round_up((int64_t)temp, 256) + 256;
+        place(4 * (size_t)round_up(ni * 4, 256) + w.sort_temp_bytes, w.sort_off, w.sort_bytes);
+    }
     place((size_t)(n_i_max + 512) * sizeof(int32_t), w.slot_off, w.slot_bytes);
     place(64, w.ctl_off, w.ctl_bytes);
     w.total = off;
@@ -126,7 +140,7 @@ struct nb_ctx {
     bool predicted = false;
     double t_pred = 0.0;
     // options
-    int64_t opt_j_split = 0, opt_i_block = 0;
+    int64_t opt_j_split = 0, opt_i_block = 0, opt_order_rows = 1;
     // last launch
     int64_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     // host path: device mirrors owned by the context
@@ -148,6 +162,7 @@ namespace {
 // ragged end, which is why several waves of short CTAs beat one wave of long ones.
 // rows split into more than kWideGatherChunks chunks are gathered by a block each, if there are few enough of them
 // that a warp per row would leave SMs idle
+constexpr int kOrderMinRows = 256;  // smaller active blocks are processed in the order given
 constexpr int kWideGatherChunks = 64;
 constexpr int64_t kWideGatherRows = 4096;
 constexpr double kPrologueJ = 48.0;
@@ -508,6 +523,42 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     const int64_t row0 = (int64_t)p.main_blocks * sh.rows;
     const bool has_split = p.n_chunks > 1 && row0 < n_i;
     int32_t* ctl = reinterpret_cast<int32_t*>(c->ws + c->lay.ctl_off);
+    // S2, first half: process the rows in Morton order of their predicted positions (order.cuh)
+    fa.perm = nullptr;
+    // ... when the force kernel is long enough for the ~7 % it gains to pay for the sort (~10 us in one CTA up to
+    // 4096 rows, ~80 us for the device-wide sort of larger blocks)
+    const double pairs = (double)n_i * (double)c->n;
+    const bool order_pays = n_i <= kSmallSort ? pairs >= 2.0e8 : pairs >= 1.5e9;
+    if (c->opt_order_rows == 2 || (c->opt_order_rows == 1 && n_i >= kOrderMinRows && order_pays)) {
+        const size_t seg = (size_t)round_up((int64_t)std::max<int64_t>(c->n_i_max, 1) * 4, 256);
+        unsigned char* sb = c->ws + c->lay.sort_off;
+        OrderArgs oa{};
+        oa.gather = reinterpret_cast<const float4*>(c->ws + c->lay.gather_off);
+        oa.i_idx = i_idx;
+        oa.n_i = n_i;
+        oa.box = reinterpret_cast<uint32_t*>(ctl + 4);
+        oa.ticket = ctl + 2;
+        oa.keys = reinterpret_cast<uint32_t*>(sb);
+        oa.rows = reinterpret_cast<int32_t*>(sb + 2 * seg);
+        if (n_i <= kSmallSort) {
+            order_small_kernel<<<1, kSmallSortThreads, 0, st>>>(oa);
+            NB_CUDA(cudaGetLastError());
+            fa.perm = oa.rows;
+            ++launches;
+        } else {
+            const unsigned blocks = (unsigned)((n_i + kOrderThreads - 1) / kOrderThreads);
+            bbox_kernel<<<std::min<unsigned>(blocks, 4u * (unsigned)c->num_sms), kOrderThreads, 0, st>>>(oa);
+            NB_CUDA(cudaGetLastError());
+            key_kernel<<<blocks, kOrderThreads, 0, st>>>(oa);
+            NB_CUDA(cudaGetLastError());
+            cub::DoubleBuffer<uint32_t> dk(oa.keys, reinterpret_cast<uint32_t*>(sb + seg));
+            cub::DoubleBuffer<int32_t> dv(oa.rows, reinterpret_cast<int32_t*>(sb + 3 * seg));
+            size_t temp = c->lay.sort_temp_bytes;
+            NB_CUDA(cub::DeviceRadixSort::SortPairs(sb + 4 * seg, temp, dk, dv, (int)n_i, 0, 30, st));
+            fa.perm = dv.Current();
+            launches += 3;  // bbox, keys, and the library sort counted as one
+        }
+    }
     fa.slot_count = reinterpret_cast<int32_t*>(c->ws + c->lay.slot_off);
     fa.overflow_ws = ctl;
     int rc = force_dispatch(variant, p.shape, nullptr, &p, &fa, st);
@@ -516,6 +567,7 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     {  // S5 + n_overflow: always launched, with no rows when nothing was split
         GatherArgs ga{};
         ga.row0 = (int32_t)(has_split ? row0 : n_i); ga.n_i = n_i; ga.n_chunks = p.n_chunks; ga.cap = c->cap;
+        ga.perm = fa.perm;
         ga.chunk_j = p.tiles_per_chunk * sh.jt;
         ga.part_sum = fa.part_sum;
         ga.acc = acc; ga.jerk = jerk; ga.pot = pot; ga.nbr_count = nbr_count; ga.nbr_list = nbr_list; ga.n_overflow = n_overflow;
@@ -649,6 +701,11 @@ int nb_set_option(nb_ctx* c, const char* key, int64_t value) {
     if (!c || !key || value < 0) return NB_E_INVAL;
     if (!strcmp(key, "j_split")) {
         c->opt_j_split = value;
+        return NB_OK;
+    }
+    if (!strcmp(key, "order_rows")) {
+        if (value > 2) return NB_E_INVAL;
+        c->opt_order_rows = value;
         return NB_OK;
     }
     if (!strcmp(key, "i_block")) {
