@@ -34,7 +34,7 @@ FLOPS_PER_PAIR = 60.0  # convention of BASELINE.json ("e.g. 60 for force+jerk"),
 LANE_SLOTS_PER_PAIR = 25.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE force_kernel launch of the default workload, from the
 # committed capture profiles/r1_force_kernel_c5_ncu_full.md (ncu --set full); None for other workloads.
-FORCE_DRAM_BYTES_C5 = 427.69e6 + 653.18e6
+FORCE_DRAM_BYTES_C5 = 1233.72e6 + 759.58e6
 METRIC = "regular-force Ginteractions/s (acc+jerk+nbr list)"
 UNIT = "Gpairs/s"
 
@@ -370,7 +370,7 @@ def run_gpu_arm(args):
                                "traffic": None, "ms": t_pred * 1e3,
                                "note": f"200 B/j algorithmic (112 read + 40 + 48 written), peak {peaks['src']} copy bandwidth; ms is the "
                                        f"interval between two events around ONE launch inside the step and includes the "
-                                       f"event-to-kernel latency (the kernel alone: 37.8 us = 5.5 TB/s in "
+                                       f"event-to-kernel latency (the kernel alone: 38.6 us = 5.4 TB/s in "
                                        f"profiles/r1_bench_c5_launches.md)"},
         "launch": info, "gpu_launches": int(info["launches"] + 1) * args.steps,
         "mean_neighbours": mean_cnt, "overflow_rows": n_over, "clocks": clocks, "e2e": e2e,
