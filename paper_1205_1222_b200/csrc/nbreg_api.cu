@@ -258,17 +258,16 @@ Plan make_plan(const Machine* c, int32_t n_i, int64_t opt_i_block, int64_t opt_j
     return best;
 }
 
-// two j-tile stages + their mbarriers
-size_t force_smem_bytes(int ipt, int warps, int jt) {
-    (void)ipt;
-    (void)warps;
-    return 2 * (size_t)jt * kBytesPerJ + 2 * sizeof(uint64_t);
+// two j-tile stages + their mbarriers + the fp64 running sums (6 per row, 7 with the potential)
+size_t force_smem_bytes(int ipt, int warps, int jt, bool pot) {
+    return 2 * (size_t)jt * kBytesPerJ + 2 * sizeof(uint64_t) +
+           (size_t)ipt * warps * 32 * (pot ? 7 : 6) * sizeof(double);
 }
 
 template <int IPT, int WARPS, int JT, int MINB, bool VEL, bool POT>
 int query_force(int* per_sm) {
     auto kern = force_kernel<IPT, WARPS, JT, MINB, VEL, POT>;
-    const size_t smem = force_smem_bytes(IPT, WARPS, JT);
+    const size_t smem = force_smem_bytes(IPT, WARPS, JT, POT);
     NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     NB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, WARPS * 32, smem));
     return NB_OK;
@@ -276,7 +275,7 @@ int query_force(int* per_sm) {
 
 template <int IPT, int WARPS, int JT, int MINB, bool VEL, bool POT>
 int launch_force(const Plan& p, const ForceArgs& fa, cudaStream_t st) {
-    const size_t smem = force_smem_bytes(IPT, WARPS, JT);
+    const size_t smem = force_smem_bytes(IPT, WARPS, JT, POT);
     force_kernel<IPT, WARPS, JT, MINB, VEL, POT><<<p.grid, WARPS * 32, smem, st>>>(fa);
     NB_CUDA(cudaGetLastError());
     return NB_OK;

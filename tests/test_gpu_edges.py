@@ -43,7 +43,7 @@ def test_shapes_and_splits_agree_bitwise_on_lists_and_closely_on_sums(oracle):
         for q in range(wl.n_i):
             c = ref["nbr_count"][q]
             assert np.array_equal(g["nbr_list"][q, :c], ref["nbr_list"][q, :c])
-        assert parity.relerr(g["acc"], ref["acc"]).max() < 5e-7
+        assert parity.relerr(g["acc"], ref["acc"]).max() < 1e-6  # two fp32 evaluations, each within ~3e-7 of fp64
 
 
 @pytest.mark.parametrize("i_block", [32, 256])
@@ -85,7 +85,7 @@ def test_degenerate_radii_and_tiny_blocks(oracle):
     # n_i = 1 and n_i = 0
     one = inputs.Workload(wl.state, wl.i_idx[20:21].copy(), wl.r_s[20:21].copy(), wl.k, wl.cap)
     g1, _ = run_gpu(one)
-    assert np.array_equal(g1["acc"][0], gpu["acc"][20]) or parity.relerr(g1["acc"], gpu["acc"][20:21]).max() < 5e-7
+    assert np.array_equal(g1["acc"][0], gpu["acc"][20]) or parity.relerr(g1["acc"], gpu["acc"][20:21]).max() < 1e-6
     _full_check(oracle, one, g1)
     zero = inputs.Workload(wl.state, wl.i_idx[:0].copy(), wl.r_s[:0].copy(), wl.k, wl.cap)
     g0, _ = run_gpu(zero)
@@ -274,8 +274,8 @@ def test_host_entry_point_in_row_chunks(oracle):
     for q in np.nonzero(ok)[0][::7]:
         c = dev_out["nbr_count"][q]
         assert np.array_equal(host["nbr_list"][q, :c], dev_out["nbr_list"][q, :c])
-    assert parity.relerr(host["acc"], dev_out["acc"]).max() < 5e-7
-    assert parity.relerr(host["jerk"], dev_out["jerk"]).max() < 5e-6
+    assert parity.relerr(host["acc"], dev_out["acc"]).max() < 1e-6  # two fp32 evaluations, each within ~3e-7 of fp64
+    assert parity.relerr(host["jerk"], dev_out["jerk"]).max() < 1e-5
     _full_check(oracle, wl, host)
     ctx.close()
 
@@ -296,7 +296,7 @@ def test_row_ordering_paths(oracle, n_i):
         for q in np.nonzero(ok)[0][:: max(1, n_i // 500)]:
             c = plain["nbr_count"][q]
             assert np.array_equal(g["nbr_list"][q, :c], plain["nbr_list"][q, :c])
-        assert parity.relerr(g["acc"], plain["acc"]).max() < 5e-7
+        assert parity.relerr(g["acc"], plain["acc"]).max() < 1e-6
     xp, vp = oracle.predict_state(wl.state)
     parity.compare(oracle, xp, vp, wl.state.m, wl.i_idx, wl.r_s, wl.cap, g, dtr=dtr, check_pot=True)
     parity.check_overflow_flag(g, wl.cap)
