@@ -34,7 +34,7 @@ FLOPS_PER_PAIR = 60.0  # convention of BASELINE.json ("e.g. 60 for force+jerk"),
 LANE_SLOTS_PER_PAIR = 25.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE force_kernel launch of the default workload, from the
 # committed capture profiles/r1_force_kernel_c5_ncu_full.md (ncu --set full); None for other workloads.
-FORCE_DRAM_BYTES_C5 = 1233.72e6 + 759.58e6
+FORCE_DRAM_BYTES_C5 = 1262.53e6 + 790.06e6
 METRIC = "regular-force Ginteractions/s (acc+jerk+nbr list)"
 UNIT = "Gpairs/s"
 
