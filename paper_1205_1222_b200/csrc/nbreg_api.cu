@@ -108,7 +108,7 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
         size_t temp = 0;
         cub::DoubleBuffer<uint32_t> dk(nullptr, nullptr);
         cub::DoubleBuffer<int32_t> dv(nullptr, nullptr);
-        cub::DeviceRadixSort::SortPairs(nullptr, temp, dk, dv, (int)ni, 0, 30);
+        cub::DeviceRadixSort::SortPairs(nullptr, temp, dk, dv, (int)ni, 0, kKeyBits);
         w.sort_temp_bytes = (size_t)round_up((int64_t)temp, 256) + 256;
         place(4 * (size_t)round_up(ni * 4, 256) + w.sort_temp_bytes, w.sort_off, w.sort_bytes);
     }
@@ -525,9 +525,9 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     // S2, first half: process the rows in Morton order of their predicted positions (order.cuh)
     fa.perm = nullptr;
     // ... when the force kernel is long enough for the ~7 % it gains to pay for the sort (~10 us in one CTA up to
-    // 4096 rows, ~80 us for the device-wide sort of larger blocks)
+    // 4096 rows, ~60 us for the device-wide sort of larger blocks)
     const double pairs = (double)n_i * (double)c->n;
-    const bool order_pays = n_i <= kSmallSort ? pairs >= 2.0e8 : pairs >= 1.5e9;
+    const bool order_pays = n_i <= kSmallSort ? pairs >= 2.0e8 : pairs >= 1.0e9;
     if (c->opt_order_rows == 2 || (c->opt_order_rows == 1 && n_i >= kOrderMinRows && order_pays)) {
         const size_t seg = (size_t)round_up((int64_t)std::max<int64_t>(c->n_i_max, 1) * 4, 256);
         unsigned char* sb = c->ws + c->lay.sort_off;
@@ -553,7 +553,7 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
             cub::DoubleBuffer<uint32_t> dk(oa.keys, reinterpret_cast<uint32_t*>(sb + seg));
             cub::DoubleBuffer<int32_t> dv(oa.rows, reinterpret_cast<int32_t*>(sb + 3 * seg));
             size_t temp = c->lay.sort_temp_bytes;
-            NB_CUDA(cub::DeviceRadixSort::SortPairs(sb + 4 * seg, temp, dk, dv, (int)n_i, 0, 30, st));
+            NB_CUDA(cub::DeviceRadixSort::SortPairs(sb + 4 * seg, temp, dk, dv, (int)n_i, 0, kKeyBits, st));
             fa.perm = dv.Current();
             launches += 3;  // bbox, keys, and the library sort counted as one
         }
