@@ -326,7 +326,10 @@ def run_gpu_arm(args):
                      nbr_list=torch.empty((wl.n_i, wl.cap), dtype=torch.int32).pin_memory(),
                      n_overflow=torch.zeros(1, dtype=torch.int32).pin_memory())
         h2d = sum(t.numel() * t.element_size() for t in h_in + [h_idx, h_rs])
-        d2h = sum(t.numel() * t.element_size() for t in h_out.values())
+        # device -> host: acc, jerk, counts, n_overflow in full; of the (n_i x cap) list array only the columns up to
+        # the longest stored list, rounded up to 32 (what nb_regular_force_host copies)
+        width = min(wl.cap, -(-int(torch.clamp(out["nbr_count"], max=wl.cap).max().item()) // 32) * 32)
+        d2h = wl.n_i * (24 + 24 + 4 + 4 * width) + 4
         ksteps = max(1, min(args.steps, 3))
         ctx.nb_regular_force_host(*h_in, h_idx, h_rs, s.t, h_out)  # warm-up (allocates the mirrors)
         if dist: dist.barrier()

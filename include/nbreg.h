@@ -133,8 +133,9 @@ int nb_irregular_force(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const int
 /* End-to-end convenience with HOST buffers: copies the j-state and the active block to device buffers the
  * context owns (allocated on first use, sized by n_max / n_i_max / nbr_cap), runs nb_set_j + nb_regular_force
  * on an internal stream -- in up to 8 row chunks, so that the copy of one chunk's outputs back to the host runs on
- * a second stream while the next chunk is computed -- and synchronises when acc, jerk, nbr_count, nbr_list
- * (n_i x nbr_cap) and n_overflow have arrived.  All pointers are host pointers with the shapes documented above. */
+ * a second stream while the next chunk is computed -- and synchronises when acc, jerk, nbr_count, nbr_list and
+ * n_overflow have arrived.  Of nbr_list only the columns that hold entries are copied (up to the longest stored
+ * list of each chunk, rounded up to 32): entries past a row's count are left untouched in the host array too.  All pointers are host pointers with the shapes documented above. */
 int nb_regular_force_host(nb_ctx* ctx, int64_t n, const double* x0, const double* v0, const double* a0,
                           const double* j0, const double* m, const double* t0, int32_t n_i, const int32_t* i_idx,
                           const double* r_s, double t, double* acc, double* jerk, int32_t* nbr_count,

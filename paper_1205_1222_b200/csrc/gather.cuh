@@ -198,4 +198,16 @@ __global__ void __launch_bounds__(kWideThreads) reduce_gather_wide_kernel(Gather
     }
 }
 
+// Longest stored list of a block of rows, max_q min(count[q], cap): lets the host entry point copy back only the
+// columns of nbr_list that hold entries.  *out must be zero on entry.
+__global__ void __launch_bounds__(256) list_width_kernel(const int32_t* nbr_count, int32_t n_rows, int32_t cap,
+                                                         int32_t* out) {
+    int32_t m = 0;
+    for (int64_t q = (int64_t)blockIdx.x * 256 + threadIdx.x; q < n_rows; q += (int64_t)gridDim.x * 256)
+        m = max(m, min(nbr_count[q], cap));
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, off));
+    if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
+}
+
 }  // namespace nbreg

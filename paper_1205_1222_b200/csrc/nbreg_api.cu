@@ -146,7 +146,7 @@ struct nb_ctx {
     // host path: device mirrors owned by the context
     cudaStream_t hstream = nullptr, hcopy = nullptr;  // compute and device-to-host copy streams
     cudaEvent_t hdone[kHostChunks] = {};              // "rows of chunk k are final"
-    int32_t* hovf = nullptr;                          // pinned: overflow count of each chunk
+    int32_t* hovf = nullptr;                          // pinned: overflow count, then longest list, of each chunk
     unsigned char* hbuf = nullptr;
     size_t hbuf_bytes = 0;
 };
@@ -627,7 +627,7 @@ int nb_regular_force_host(nb_ctx* c, int64_t n, const double* x0, const double* 
     if (!c->hcopy) NB_CUDA(cudaStreamCreateWithFlags(&c->hcopy, cudaStreamNonBlocking));
     for (int k = 0; k < kHostChunks; ++k)
         if (!c->hdone[k]) NB_CUDA(cudaEventCreateWithFlags(&c->hdone[k], cudaEventDisableTiming));
-    if (!c->hovf) NB_CUDA(cudaMallocHost(&c->hovf, kHostChunks * sizeof(int32_t)));
+    if (!c->hovf) NB_CUDA(cudaMallocHost(&c->hovf, 2 * kHostChunks * sizeof(int32_t)));
     // device mirrors, carved from one allocation sized for n_max / n_i_max / cap
     const size_t nmax = (size_t)c->n_max, imax = (size_t)c->n_i_max;
     size_t off = 0;
@@ -668,24 +668,39 @@ int nb_regular_force_host(nb_ctx* c, int64_t n, const double* x0, const double* 
     rows_per_chunk = round_up(rows_per_chunk, 1024);
     if (!overlap_pays) rows_per_chunk = round_up(std::max<int64_t>(n_i, 1), 1024);
     const int n_chunks = n_i > 0 ? (int)((n_i + rows_per_chunk - 1) / rows_per_chunk) : 1;
+    // first everything that computes, then, chunk by chunk as they finish, the copies: only the columns of nbr_list
+    // that hold entries travel (the longest stored list of the chunk, rounded up to 32 columns)
+    int32_t* d_ovf = (int32_t*)(b + o_ovf);          // [kHostChunks] overflow counts
+    int32_t* d_wid = d_ovf + kHostChunks;            // [kHostChunks] longest stored lists
+    NB_CUDA(cudaMemsetAsync(d_wid, 0, kHostChunks * sizeof(int32_t), st));
     for (int k = 0; k < n_chunks; ++k) {
         const size_t r0 = (size_t)k * (size_t)rows_per_chunk;
         const size_t nr = n_i > 0 ? std::min<size_t>((size_t)rows_per_chunk, ni - r0) : 0;
-        int32_t* d_ovf = (int32_t*)(b + o_ovf) + k;
         rc = nb_regular_force(c, (int32_t)nr, (const int32_t*)(b + o_idx) + r0, (const double*)(b + o_rs) + r0, t,
                               (double*)(b + o_acc) + 3 * r0, (double*)(b + o_jrk) + 3 * r0, (int32_t*)(b + o_cnt) + r0,
-                              (int32_t*)(b + o_lst) + r0 * cap, d_ovf, st);
+                              (int32_t*)(b + o_lst) + r0 * cap, d_ovf + k, st);
         if (rc != NB_OK) return rc;
-        NB_CUDA(cudaEventRecord(c->hdone[k], st));
-        NB_CUDA(cudaStreamWaitEvent(cs, c->hdone[k], 0));
         if (nr > 0) {
-            NB_CUDA(cudaMemcpyAsync(acc + 3 * r0, (double*)(b + o_acc) + 3 * r0, nr * 24, cudaMemcpyDeviceToHost, cs));
-            NB_CUDA(cudaMemcpyAsync(jerk + 3 * r0, (double*)(b + o_jrk) + 3 * r0, nr * 24, cudaMemcpyDeviceToHost, cs));
-            NB_CUDA(cudaMemcpyAsync(nbr_count + r0, (int32_t*)(b + o_cnt) + r0, nr * 4, cudaMemcpyDeviceToHost, cs));
-            NB_CUDA(cudaMemcpyAsync(nbr_list + r0 * cap, (int32_t*)(b + o_lst) + r0 * cap, nr * cap * 4,
-                                    cudaMemcpyDeviceToHost, cs));
+            const unsigned blocks = (unsigned)std::min<size_t>((nr + 255) / 256, 1024);
+            list_width_kernel<<<blocks, 256, 0, st>>>((const int32_t*)(b + o_cnt) + r0, (int32_t)nr, c->cap, d_wid + k);
+            NB_CUDA(cudaGetLastError());
         }
-        NB_CUDA(cudaMemcpyAsync(c->hovf + k, d_ovf, sizeof(int32_t), cudaMemcpyDeviceToHost, cs));
+        NB_CUDA(cudaMemcpyAsync(c->hovf + k, d_ovf + k, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        NB_CUDA(cudaMemcpyAsync(c->hovf + kHostChunks + k, d_wid + k, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        NB_CUDA(cudaEventRecord(c->hdone[k], st));
+    }
+    for (int k = 0; k < n_chunks; ++k) {
+        const size_t r0 = (size_t)k * (size_t)rows_per_chunk;
+        const size_t nr = n_i > 0 ? std::min<size_t>((size_t)rows_per_chunk, ni - r0) : 0;
+        NB_CUDA(cudaEventSynchronize(c->hdone[k]));  // chunk k is final on the device, its list width is known
+        if (nr == 0) continue;
+        NB_CUDA(cudaMemcpyAsync(acc + 3 * r0, (double*)(b + o_acc) + 3 * r0, nr * 24, cudaMemcpyDeviceToHost, cs));
+        NB_CUDA(cudaMemcpyAsync(jerk + 3 * r0, (double*)(b + o_jrk) + 3 * r0, nr * 24, cudaMemcpyDeviceToHost, cs));
+        NB_CUDA(cudaMemcpyAsync(nbr_count + r0, (int32_t*)(b + o_cnt) + r0, nr * 4, cudaMemcpyDeviceToHost, cs));
+        const size_t width = std::min<size_t>(cap, (size_t)round_up(c->hovf[kHostChunks + k], 32));
+        if (width > 0)
+            NB_CUDA(cudaMemcpy2DAsync(nbr_list + r0 * cap, cap * 4, (int32_t*)(b + o_lst) + r0 * cap, cap * 4, width * 4,
+                                      nr, cudaMemcpyDeviceToHost, cs));
     }
     NB_CUDA(cudaStreamSynchronize(st));
     NB_CUDA(cudaStreamSynchronize(cs));
