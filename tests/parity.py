@@ -88,25 +88,35 @@ def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None
             continue
         # every disagreeing j must sit inside the boundary band
         i = sub_idx[q]
-        if cnt_g[q] > cap and not diff:
-            # counts differ on an overflowed row: cannot name the pair; bound the number of band pairs instead
+        if cnt_g[q] > cap:
+            # Overflowed row: the stored list is cut at cap.  Entries the GPU lists and the oracle sums are named
+            # (diff) and must be band pairs; what the count difference leaves unexplained are band pairs that did not
+            # make it into the stored list: the best-fitting ones are moved across.  The oracle's sums are adjusted
+            # accordingly (H4: a row with a band pair is force-checked with the GPU's own classification).
             d = _rmin(xp, vp, i, np.arange(xp.shape[0]), sub_dt[q])
-            nband = int((np.abs(d - sub_rs[q]) < BAND * sub_rs[q]).sum())
-            delta = int(cnt_o[q]) - int(cnt_g[q])  # > 0: the GPU summed `delta` pairs the oracle listed
-            assert abs(delta) <= nband, f"row {rows[q]}: overflow count mismatch"
-            n_band_pairs += abs(delta)
-            # the stored list is cut at cap, so the flipped pairs cannot be read off it: they are band pairs on the
-            # oracle's neighbour side (delta > 0) or summed side (delta < 0); move the best-fitting `|delta|` of them
-            band = np.nonzero(np.abs(d - sub_rs[q]) < BAND * sub_rs[q])[0]
-            cand = [int(j) for j in band if j != i and ((d[j] < sub_rs[q]) == (delta > 0))]
+            in_band = np.abs(d - sub_rs[q]) < BAND * sub_rs[q]
+            for j in diff:
+                assert in_band[j], f"row {rows[q]} (i={i}): list differs at j={j} outside the band"
+            if diff:
+                da, dj, dp = _pair_terms(xp, vp, m, i, np.array(sorted(diff)))
+                acc_o[q] -= da
+                jerk_o[q] -= dj
+                if ex:
+                    pot_o[q] -= dp
+            delta = int(cnt_o[q]) + len(diff) - int(cnt_g[q])  # > 0: the GPU summed `delta` pairs the oracle listed
+            n_band_pairs += len(diff) + abs(delta)
+            cand = [int(j) for j in np.nonzero(in_band)[0]
+                    if j != i and j not in diff and j not in set_g and ((d[j] < sub_rs[q]) == (delta > 0))]
+            assert abs(delta) <= len(cand), f"row {rows[q]}: overflow count mismatch"
             best = None
-            for combo in itertools.islice(itertools.combinations(cand, abs(delta)), 256):
-                da, dj, dp = _pair_terms(xp, vp, m, i, np.array(combo))
-                sign = 1.0 if delta > 0 else -1.0
-                trial = acc_o[q] + sign * da
-                err = np.linalg.norm(acc_g[q] - trial)
-                if best is None or err < best[0]:
-                    best = (err, trial, jerk_o[q] + sign * dj, sign * dp)
+            if delta != 0:
+                for combo in itertools.islice(itertools.combinations(cand, abs(delta)), 256):
+                    da, dj, dp = _pair_terms(xp, vp, m, i, np.array(combo))
+                    sign = 1.0 if delta > 0 else -1.0
+                    trial = acc_o[q] + sign * da
+                    err = np.linalg.norm(acc_g[q] - trial)
+                    if best is None or err < best[0]:
+                        best = (err, trial, jerk_o[q] + sign * dj, sign * dp)
             if best is not None:
                 acc_o[q], jerk_o[q] = best[1], best[2]
                 if ex:
