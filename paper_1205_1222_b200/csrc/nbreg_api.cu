@@ -383,6 +383,13 @@ int nb_create(nb_ctx** out, int device, int64_t n_max, int64_t n_i_max, int32_t 
         delete c;
         return cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(reduce_gather_wide_kernel)");
     }
+    if (cudaFuncSetAttribute(order_small_kernel<512, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)OrderSmall<512, 8>::smem_bytes) != cudaSuccess ||
+        cudaFuncSetAttribute(order_small_kernel<1024, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)OrderSmall<1024, 8>::smem_bytes) != cudaSuccess) {
+        delete c;
+        return cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(order_small_kernel)");
+    }
     for (int v = 0; v < 4; ++v) {
         for (int k = 0; k < kNumShapes; ++k) {
             const int rc = force_dispatch(v, k, &c->ctas_per_sm[v][k], nullptr, nullptr, nullptr);
@@ -524,8 +531,8 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     int32_t* ctl = reinterpret_cast<int32_t*>(c->ws + c->lay.ctl_off);
     // S2, first half: process the rows in Morton order of their predicted positions (order.cuh)
     fa.perm = nullptr;
-    // ... when the force kernel is long enough for the ~7 % it gains to pay for the sort (~10 us in one CTA up to
-    // 4096 rows, ~60 us for the device-wide sort of larger blocks)
+    // ... when the force kernel is long enough for the 2-7 % it gains to pay for the sort (~10 us in one CTA up to
+    // 8192 rows, ~60 us for the device-wide sort of larger blocks)
     const double pairs = (double)n_i * (double)c->n;
     const bool order_pays = n_i <= kSmallSort ? pairs >= 2.0e8 : pairs >= 1.0e9;
     if (c->opt_order_rows == 2 || (c->opt_order_rows == 1 && n_i >= kOrderMinRows && order_pays)) {
@@ -540,7 +547,10 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         oa.keys = reinterpret_cast<uint32_t*>(sb);
         oa.rows = reinterpret_cast<int32_t*>(sb + 2 * seg);
         if (n_i <= kSmallSort) {
-            order_small_kernel<<<1, kSmallSortThreads, 0, st>>>(oa);
+            if (n_i <= 4096)
+                order_small_kernel<512, 8><<<1, 512, OrderSmall<512, 8>::smem_bytes, st>>>(oa);
+            else
+                order_small_kernel<1024, 8><<<1, 1024, OrderSmall<1024, 8>::smem_bytes, st>>>(oa);
             NB_CUDA(cudaGetLastError());
             fa.perm = oa.rows;
             ++launches;

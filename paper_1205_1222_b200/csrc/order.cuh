@@ -23,8 +23,8 @@
 
 namespace nbreg {
 
-constexpr int kSmallSort = 4096;      // rows the one-CTA sort handles
-constexpr int kSmallSortThreads = 512;
+constexpr int kSmallSort = 8192;      // rows the one-CTA sort handles
+constexpr int kSmallSortRadixBits = 5;  // 24-bit keys in five passes (measured: 4 bits +1 %, 6 bits equal)
 constexpr int kOrderThreads = 256;
 
 struct OrderArgs {
@@ -74,28 +74,32 @@ __device__ __forceinline__ void box_scale(const uint32_t box[6], float lo[3], fl
     }
 }
 
-// ---- small blocks: everything in one CTA (box, keys, block-wide radix sort of (key, row) pairs from the library)
-__global__ void __launch_bounds__(kSmallSortThreads) order_small_kernel(OrderArgs a) {
-    constexpr int kItems = kSmallSort / kSmallSortThreads;
-    using BlockSort = cub::BlockRadixSort<uint32_t, kSmallSortThreads, kItems, int32_t>;
-    __shared__ typename BlockSort::TempStorage sort_storage;
+// ---- small blocks: everything in one CTA (box, keys, block-wide radix sort of (key, row) pairs from the library).
+// Two sizes: 512 threads x 8 rows and 1024 x 8 (measured at N = 65536: 1024 x 16 loses to the device-wide sort at
+// 16384 rows, 1.149 against 1.134 ms per call).  The sort's temporary storage goes to dynamic shared memory.
+template <int THREADS, int ITEMS>
+struct OrderSmall {
+    using BlockSort = cub::BlockRadixSort<uint32_t, THREADS, ITEMS, int32_t, kSmallSortRadixBits>;
+    static constexpr size_t smem_bytes = sizeof(typename BlockSort::TempStorage);
+};
+
+template <int THREADS, int ITEMS>
+__global__ void __launch_bounds__(THREADS) order_small_kernel(OrderArgs a) {
+    using BlockSort = typename OrderSmall<THREADS, ITEMS>::BlockSort;
+    extern __shared__ __align__(16) unsigned char order_smem[];
+    typename BlockSort::TempStorage& sort_storage = *reinterpret_cast<typename BlockSort::TempStorage*>(order_smem);
     __shared__ uint32_t box[6];
     const int tid = threadIdx.x;
     if (tid < 6) box[tid] = 0u;
     __syncthreads();
-    float3 p[kItems];
     uint32_t m[6] = {0u, 0u, 0u, 0u, 0u, 0u};
+    for (int q = tid; q < a.n_i; q += THREADS) {
+        const float3 p = row_position(a, q);
+        const uint32_t o[3] = {ordered(p.x), ordered(p.y), ordered(p.z)};
 #pragma unroll
-    for (int k = 0; k < kItems; ++k) {
-        const int q = tid * kItems + k;  // blocked arrangement
-        if (q < a.n_i) {
-            p[k] = row_position(a, q);
-            const uint32_t o[3] = {ordered(p[k].x), ordered(p[k].y), ordered(p[k].z)};
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                m[c] = max(m[c], o[c]);
-                m[3 + c] = max(m[3 + c], ~o[c]);
-            }
+        for (int c = 0; c < 3; ++c) {
+            m[c] = max(m[c], o[c]);
+            m[3 + c] = max(m[3 + c], ~o[c]);
         }
     }
 #pragma unroll
@@ -110,18 +114,22 @@ __global__ void __launch_bounds__(kSmallSortThreads) order_small_kernel(OrderArg
     __syncthreads();
     float lo[3], scale[3];
     box_scale(box, lo, scale);
-    uint32_t key[kItems];
-    int32_t row[kItems];
+    uint32_t key[ITEMS];
+    int32_t row[ITEMS];
 #pragma unroll
-    for (int k = 0; k < kItems; ++k) {
-        const int q = tid * kItems + k;
-        key[k] = (q < a.n_i) ? morton_key(p[k].x, p[k].y, p[k].z, lo, scale) : (1u << kKeyBits);  // padding sorts last
+    for (int k = 0; k < ITEMS; ++k) {
+        const int q = tid * ITEMS + k;  // blocked arrangement: a stable sort keeps equal keys in row order
+        key[k] = (1u << kKeyBits) - 1u;  // padding: the largest key; the sort is stable and padding has the largest q, so it stays last
+        if (q < a.n_i) {
+            const float3 p = row_position(a, q);  // second read of the record: an L2 hit, cheaper than 3 registers per row
+            key[k] = morton_key(p.x, p.y, p.z, lo, scale);
+        }
         row[k] = q;
     }
-    BlockSort(sort_storage).Sort(key, row, 0, kKeyBits + 1);  // bit 24 is set only in the padding keys
+    BlockSort(sort_storage).Sort(key, row, 0, kKeyBits);
 #pragma unroll
-    for (int k = 0; k < kItems; ++k) {
-        const int q = tid * kItems + k;
+    for (int k = 0; k < ITEMS; ++k) {
+        const int q = tid * ITEMS + k;
         if (q < a.n_i) a.rows[q] = row[k];
     }
 }

@@ -297,10 +297,10 @@ def test_host_entry_point_in_row_chunks(oracle):
     ctx.close()
 
 
-@pytest.mark.parametrize("n_i", [300, 4096, 4097, 9001])
+@pytest.mark.parametrize("n_i", [300, 4096, 4097, 8192, 9001])
 def test_row_ordering_paths(oracle, n_i):
-    """Rows processed in Morton order of the predicted positions (one-CTA sort up to 4096 rows, device-wide sort
-    above): outputs land in the caller's rows; lists and counts identical to the unordered run, sums to rounding."""
+    """Rows processed in Morton order of the predicted positions (one-CTA sorts of 512 x 8 and 1024 x 8 rows, device-wide
+    sort above 8192): outputs land in the caller's rows; lists and counts identical to the unordered run, sums to rounding."""
     wl = _wl(oracle, 3001, n_i, 24, 64, masses="salpeter")
     wl.i_idx[5] = wl.i_idx[4]  # duplicates keep their own rows
     wl.r_s[5] = wl.r_s[4]
