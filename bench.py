@@ -252,6 +252,14 @@ def run_gpu_arm(args):
     dev = torch.device(f"cuda:{local}")
     peaks = _peaks()
     wl = build_workload(args.config, args.n_i)  # every rank: the same seeded workload (independent replicas)
+    job_pairs, job_replicas, shard_rows = wl.pairs, world, None
+    if args.shard == "rows":  # ONE job, its rows split over the ranks (strong scaling); no data-path collective
+        import dataclasses
+        from paper_1205_1222_b200 import sharding
+        shard_rows = sharding.row_shard(wl.n_i, rank, world)
+        job_replicas = 1
+        wl = dataclasses.replace(wl, i_idx=np.ascontiguousarray(wl.i_idx[shard_rows[0]:shard_rows[1]]),
+                                 r_s=np.ascontiguousarray(wl.r_s[shard_rows[0]:shard_rows[1]]))
     s = wl.state
     ctx = binding.Context(s.n, wl.n_i, wl.cap, device=local)
     state_dev = ctx.set_state(s)
@@ -288,7 +296,7 @@ def run_gpu_arm(args):
     t_pred = sum(e[0].elapsed_time(e[1]) for e in evs) / 1e3 / args.steps
     t_force = sum(e[1].elapsed_time(e[2]) for e in evs) / 1e3 / args.steps
     t_max = max_over_ranks(t_step, dist, dev)
-    value = whole_job_rate(wl.pairs, args.steps, world, t_max)
+    value = whole_job_rate(job_pairs, args.steps, job_replicas, t_max)
     n_over = int(out["n_overflow"].item())
     mean_cnt = float(out["nbr_count"].double().mean().item())
 
@@ -339,7 +347,7 @@ def run_gpu_arm(args):
             ctx.nb_regular_force_host(*h_in, h_idx, h_rs, s.t, h_out)  # synchronises internally
         te = time.perf_counter() - t0
         te_max = max_over_ranks(te, dist, dev)
-        e2e = {"value": whole_job_rate(wl.pairs, ksteps, world, te_max), "unit": UNIT,
+        e2e = {"value": whole_job_rate(job_pairs, ksteps, job_replicas, te_max), "unit": UNIT,
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "steps": ksteps,
                "ms_per_step": te_max / ksteps * 1e3, "api": "nb_regular_force_host (pinned host buffers)"}
         ctx.nb_set_j(*state_dev)
@@ -354,7 +362,7 @@ def run_gpu_arm(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "scaling": "strong" if shard_rows else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": workload_config(wl, args.config),
         "fp32_peak_fraction": value / world * 1e9 * FLOPS_PER_PAIR / (peak_tf * 1e12),
         "roofline": {"bound": "alu", "kernel": "force_kernel", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
@@ -379,6 +387,10 @@ def run_gpu_arm(args):
         "mean_neighbours": mean_cnt, "overflow_rows": n_over, "clocks": clocks, "e2e": e2e,
         "next_irregular": irr,
     }
+    if shard_rows:
+        line["config"]["parallelism"] = f"rows sharded over {world} ranks (rank 0 owns rows {shard_rows[0]}..{shard_rows[1]}); " \
+                                        "every rank predicts all j; no data-path collective"
+        line["config"]["job_pairs_per_step"] = job_pairs
     if not args.no_cpu and world >= 1:
         cb, _ = cpu_baseline(wl, target_seconds=args.cpu_seconds)
         line["cpu_baseline"] = cb
@@ -400,6 +412,8 @@ def main():
     ap.add_argument("--no-irregular", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="config 3 active-block sweep 32 ... 65536 (one JSON line)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--shard", default="none", choices=["none", "rows"],
+                    help="none: N independent replicas (default, weak); rows: one job, rows split over the ranks (strong)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
