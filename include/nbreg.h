@@ -130,6 +130,56 @@ int nb_irregular_force(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const int
                        const int32_t* nbr_list, int32_t list_stride, double t, double* acc, double* jerk,
                        void* stream);
 
+/* Step (vii), PAPER.md:110 ("Execute the regular corrector.  Since the neighbour list L_i has been updated, the
+ * force polynomials should be corrected to reflect the difference between the old and new list"), and the
+ * neighbour-radius update eq. (1), for the n_i rows of a regular step that ends at time t.  The paper
+ * prints no corrector formula; readings R16-R18 of DESIGN.md state what is computed, per row q, i = i_idx[q]:
+ *   1. f1, fd1 = acc, jerk + sum_{j in L_new} f_ij - sum_{j in L_old} f_ij: the regular force and its derivative at
+ *      t with respect to the OLD list (the one the step was integrated with); f_ij = the pair terms of eq. (7), (8) on
+ *      the state predicted to t (predicted first if t differs from the last prediction), fp32 on two-float
+ *      differences, summed in fp64;
+ *   2. the cubic Hermite polynomial F(tau) through (fr0, frd0) at tau = 0 and (f1, fd1) at tau = dt_r:
+ *      d3 = F''' = [12 (fr0 - f1) + 6 dt (frd0 + fd1)] / dt^3,  d2 = F''(dt_r) = [-6 (fr0 - f1) - dt (4 frd0 + 2 fd1)] /
+ *      dt^2 + dt d3 (physical derivatives, at the END of the step), and the terms the predictor left out:
+ *      dx = F''(0) dt^4/24 + F''' dt^5/120,  dv = F''(0) dt^3/6 + F''' dt^4/24  (to be ADDED to the predicted x, v);
+ *   3. r_s_new = r_s (n_p / max(nbr_count, 1))^(1/3)   (eq. (1); nbr_count is the TRUE count of the new list).
+ * All pointers are dev pointers owned by the caller; [n_i][3] arrays are row-major double.
+ *   i_idx       int32[n_i]                 dt_r     double[n_i], > 0 (0 gives inf/nan in that row, no error)
+ *   fr0, frd0   double[n_i][3]  regular force and derivative at the START of the step (old list)
+ *   acc, jerk   double[n_i][3]  regular force and derivative at t, NEW list (outputs of nb_regular_force)
+ *   nbr_count, nbr_list, list_stride    the new list (outputs of nb_regular_force, list_stride = nbr_cap)
+ *   old_count, old_list, old_stride     the list of the step that ends; min(count, stride) entries of each list
+ *                                       are used: for a row that overflowed in either list f1, fd1 miss the entries
+ *                                       that were dropped (flagged by count > stride, as everywhere)
+ *   r_s, n_p    double[n_i]     old radius and predicted neighbour number; both NULL skips step 3
+ *   f1, fd1, d2, d3, dx, dv     double[n_i][3] outputs;   r_s_new  double[n_i] output or NULL
+ * Enqueues one kernel (plus the predictor if needed) on `stream`.  NB_E_INVAL for a null required pointer, a
+ * stride < 1 or n_i out of range; NB_E_STATE before nb_set_j. */
+typedef struct nb_corrector_io {
+    const int32_t* i_idx;
+    const double* dt_r;
+    const double* fr0;
+    const double* frd0;
+    const double* acc;
+    const double* jerk;
+    const int32_t* nbr_count;
+    const int32_t* nbr_list;
+    const int32_t* old_count;
+    const int32_t* old_list;
+    const double* r_s;
+    const double* n_p;
+    double* f1;
+    double* fd1;
+    double* d2;
+    double* d3;
+    double* dx;
+    double* dv;
+    double* r_s_new;
+    int32_t list_stride;
+    int32_t old_stride;
+} nb_corrector_io;
+int nb_regular_correct(nb_ctx* ctx, int32_t n_i, const nb_corrector_io* io, double t, void* stream);
+
 /* End-to-end convenience with HOST buffers: copies the j-state and the active block to device buffers the
  * context owns (allocated on first use, sized by n_max / n_i_max / nbr_cap), runs nb_set_j + nb_regular_force
  * on an internal stream -- in up to 8 row chunks, so that the copy of one chunk's outputs back to the host runs on

@@ -50,12 +50,21 @@ def load(build_if_missing: bool = True):
     lib.nb_regular_force.argtypes = [vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp, vp]
     lib.nb_regular_force_ex.argtypes = [vp, i32, vp, vp, vp, dbl, vp, vp, vp, vp, vp, vp, vp]
     lib.nb_irregular_force.argtypes = [vp, i32, vp, vp, vp, i32, dbl, vp, vp, vp]
+    lib.nb_regular_correct.argtypes = [vp, i32, ctypes.POINTER(CorrectorIO), dbl, vp]
     lib.nb_regular_force_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp]
     lib.nb_set_option.argtypes = [vp, ctypes.c_char_p, i64]
     lib.nb_last_launch_info.argtypes = [vp, ctypes.POINTER(i64)]
     lib.nb_plan.argtypes = [i64, i32, i32, ctypes.POINTER(i32), i64, i64, ctypes.POINTER(i64)]
     _lib = lib
     return lib
+
+
+class CorrectorIO(ctypes.Structure):
+    """nb_corrector_io of include/nbreg.h, field for field."""
+    _fields_ = [(k, ctypes.c_void_p) for k in (
+        "i_idx", "dt_r", "fr0", "frd0", "acc", "jerk", "nbr_count", "nbr_list", "old_count", "old_list", "r_s", "n_p",
+        "f1", "fd1", "d2", "d3", "dx", "dv", "r_s_new")] + [("list_stride", ctypes.c_int32),
+                                                             ("old_stride", ctypes.c_int32)]
 
 
 def _check(rc: int):
@@ -194,6 +203,29 @@ class Context:
             self._h, n_i, _dev(i_idx, torch.int32, "i_idx"), _dev(nbr_count, torch.int32, "nbr_count"),
             _dev(nbr_list, torch.int32, "nbr_list"), stride, float(t),
             _dev(out["acc"], torch.float64, "acc"), _dev(out["jerk"], torch.float64, "jerk"), _stream_ptr(stream)))
+        return out
+
+    # -- nb_regular_correct: step (vii) and eq. (1)
+    def nb_regular_correct(self, i_idx, dt_r, fr0, frd0, acc, jerk, nbr_count, nbr_list, old_count, old_list, t: float,
+                           r_s=None, n_p=None, out=None, stream=None):
+        n_i = int(i_idx.shape[0])
+        dev = self.workspace.device
+        f64 = torch.float64
+        if out is None:
+            out = {k: torch.empty((n_i, 3), dtype=f64, device=dev) for k in ("f1", "fd1", "d2", "d3", "dx", "dv")}
+            if r_s is not None:
+                out["r_s_new"] = torch.empty(n_i, dtype=f64, device=dev)
+        io = CorrectorIO()
+        for key, ten, dt in (("i_idx", i_idx, torch.int32), ("dt_r", dt_r, f64), ("fr0", fr0, f64),
+                             ("frd0", frd0, f64), ("acc", acc, f64), ("jerk", jerk, f64),
+                             ("nbr_count", nbr_count, torch.int32), ("nbr_list", nbr_list, torch.int32),
+                             ("old_count", old_count, torch.int32), ("old_list", old_list, torch.int32),
+                             ("r_s", r_s, f64), ("n_p", n_p, f64)) + tuple(
+                                 (k, out.get(k), f64) for k in ("f1", "fd1", "d2", "d3", "dx", "dv", "r_s_new")):
+            setattr(io, key, None if ten is None else _dev(ten, dt, key))
+        io.list_stride = int(nbr_list.shape[1]) if nbr_list.dim() == 2 else 1
+        io.old_stride = int(old_list.shape[1]) if old_list.dim() == 2 else 1
+        _check(self.lib.nb_regular_correct(self._h, n_i, ctypes.byref(io), float(t), _stream_ptr(stream)))
         return out
 
     # -- nb_regular_force_host (all tensors on the CPU; pinned memory recommended)

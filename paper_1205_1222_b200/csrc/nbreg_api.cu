@@ -14,6 +14,7 @@
 #include "force.cuh"
 #include "gather.cuh"
 #include "irregular.cuh"
+#include "corrector.cuh"
 #include "order.cuh"
 #include "nbreg_common.cuh"
 #include "predict.cuh"
@@ -621,6 +622,39 @@ int nb_irregular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const int32
     ia.acc = acc; ia.jerk = jerk;
     const unsigned blocks = (unsigned)((n_i + kIrrWarps - 1) / kIrrWarps);
     irregular_kernel<<<blocks, kIrrWarps * 32, 0, st>>>(ia);
+    NB_CUDA(cudaGetLastError());
+    return NB_OK;
+}
+
+int nb_regular_correct(nb_ctx* c, int32_t n_i, const nb_corrector_io* io, double t, void* stream) {
+    if (!c || !io) return NB_E_INVAL;
+    if (n_i < 0 || n_i > c->n_i_max || io->list_stride < 1 || io->old_stride < 1) return NB_E_INVAL;
+    if (n_i > 0 && (!io->i_idx || !io->dt_r || !io->fr0 || !io->frd0 || !io->acc || !io->jerk || !io->nbr_count ||
+                    !io->nbr_list || !io->old_count || !io->old_list || !io->f1 || !io->fd1 || !io->d2 || !io->d3 ||
+                    !io->dx || !io->dv))
+        return NB_E_INVAL;
+    if (io->r_s_new && (!io->r_s || !io->n_p)) return NB_E_INVAL;
+    if (c->n < 1) return NB_E_STATE;
+    NB_CUDA(cudaSetDevice(c->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (!c->predicted || c->t_pred != t) {
+        int rc = nb_predict_j(c, t, stream);
+        if (rc != NB_OK) return rc;
+    }
+    if (n_i == 0) return NB_OK;
+    CorrectorArgs ca{};
+    ca.gather = reinterpret_cast<const float4*>(c->ws + c->lay.gather_off);
+    ca.n = (int32_t)c->n;
+    ca.n_i = n_i;
+    ca.i_idx = io->i_idx; ca.dt_r = io->dt_r; ca.fr0 = io->fr0; ca.frd0 = io->frd0;
+    ca.acc = io->acc; ca.jerk = io->jerk;
+    ca.new_count = io->nbr_count; ca.new_list = io->nbr_list; ca.new_stride = io->list_stride;
+    ca.old_count = io->old_count; ca.old_list = io->old_list; ca.old_stride = io->old_stride;
+    ca.r_s = io->r_s; ca.n_p = io->n_p;
+    ca.f1 = io->f1; ca.fd1 = io->fd1; ca.d2 = io->d2; ca.d3 = io->d3; ca.dx = io->dx; ca.dv = io->dv;
+    ca.r_s_new = io->r_s_new;
+    const unsigned blocks = (unsigned)((n_i + kIrrWarps - 1) / kIrrWarps);
+    corrector_kernel<<<blocks, kIrrWarps * 32, 0, st>>>(ca);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }
