@@ -322,6 +322,40 @@ def run_gpu_arm(args):
                "note": "eq. (7), (8) over the neighbour lists of the last step; one 48 B particle-major record gathered per pair "
                        "(L2-resident at this N); bound by the L1/TEX sector rate for scattered accesses (profiles/), for which no measured peak exists in MEASURED_PEAKS.json, so no fraction is given"}
 
+    # ---- step (vii) and eq. (1): the regular corrector on the lists of two regular-force calls
+    # (radii of the second scaled by a seeded factor in [0.9, 1.1]).  Reported beside the headline, not part of it.
+    cor = None
+    if not args.no_irregular:
+        rng = np.random.default_rng(12345)
+        fac = torch.from_numpy(rng.uniform(0.9, 1.1, size=wl.n_i)).to(dev)
+        old = ctx.nb_regular_force(i_idx, r_s * fac, s.t)
+        f64 = dict(dtype=torch.float64, device=dev)
+        dt_r = torch.from_numpy(2.0 ** -rng.integers(3, 9, size=wl.n_i).astype(np.float64)).to(dev)
+        fr0, frd0 = torch.randn((wl.n_i, 3), **f64), torch.randn((wl.n_i, 3), **f64)
+        n_p = torch.full((wl.n_i,), float(wl.k), **f64)
+        cargs = (i_idx, dt_r, fr0, frd0, out["acc"], out["jerk"], out["nbr_count"], out["nbr_list"],
+                 old["nbr_count"], old["nbr_list"], s.t)
+        c_out = None
+        for _ in range(3):
+            c_out = ctx.nb_regular_correct(*cargs, r_s=r_s, n_p=n_p, out=c_out)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for _ in range(5):
+            ctx.nb_regular_correct(*cargs, r_s=r_s, n_p=n_p, out=c_out)
+        ev[1].record()
+        torch.cuda.synchronize()
+        t_cor = ev[0].elapsed_time(ev[1]) / 5 / 1e3
+        n_old = int(torch.clamp(old["nbr_count"], max=wl.cap).sum().item())
+        n_new = int(torch.clamp(out["nbr_count"], max=wl.cap).sum().item())
+        cor_bytes = (n_old + n_new) * 4 + wl.n_i * (4 * 24 + 8 * 3 + 4 * 3 + 6 * 24 + 8)
+        cor = {"kernel": "corrector_kernel", "rows": wl.n_i, "ms": t_cor * 1e3, "rows_per_s": wl.n_i / t_cor,
+               "list_entries_compared": n_old + n_new, "stream_gb_per_s": cor_bytes / t_cor / 1e9,
+               "note": "step (vii) + eq. (1): symmetric difference of the old and new list by warp-shuffle compares, pair "
+                       "terms of the members that changed, fp64 Hermite arithmetic; stream_gb_per_s counts both lists "
+                       "and the per-row arrays once (the gathers of the changed members come on top)"}
+        del old
+
     # ---- e2e: C-ABI call with HOST (pinned) buffers, copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -386,6 +420,7 @@ def run_gpu_arm(args):
         "launch": info, "gpu_launches": int(info["launches"] + 1) * args.steps,
         "mean_neighbours": mean_cnt, "overflow_rows": n_over, "clocks": clocks, "e2e": e2e,
         "next_irregular": irr,
+        "next_corrector": cor,
     }
     if shard_rows:
         line["config"]["parallelism"] = f"rows sharded over {world} ranks (rank 0 owns rows {shard_rows[0]}..{shard_rows[1]}); " \

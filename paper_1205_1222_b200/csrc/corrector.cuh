@@ -83,6 +83,24 @@ __device__ __forceinline__ bool in_list(int32_t j, const int32_t* list, int32_t 
     return found;
 }
 
+// The same question for a list in strictly ascending order (what nb_regular_force writes, R11): binary search,
+// <= log2(len) + 1 loads per lane from a row that sits in L1 after its first pass, against len shuffles.
+__device__ __forceinline__ bool in_sorted_list(int32_t j, const int32_t* list, int32_t len) {
+    int32_t lo = 0, hi = len;
+    while (lo < hi) {
+        const int32_t mid = (lo + hi) >> 1;
+        if (list[mid] < j) lo = mid + 1; else hi = mid;
+    }
+    return lo < len && list[lo] == j;
+}
+
+// Is list[0, len) strictly ascending?  (warp-uniform result)
+__device__ __forceinline__ bool is_ascending(const int32_t* list, int32_t len, int lane) {
+    bool ok = true;
+    for (int32_t e = lane; e + 1 < len; e += 32) ok &= list[e] < list[e + 1];
+    return __all_sync(0xffffffffu, ok);
+}
+
 __global__ void __launch_bounds__(kIrrWarps * 32) corrector_kernel(CorrectorArgs a) {
     const int lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * kIrrWarps + (threadIdx.x >> 5);
@@ -96,15 +114,18 @@ __global__ void __launch_bounds__(kIrrWarps * 32) corrector_kernel(CorrectorArgs
     const int32_t* lold = a.old_list + (size_t)row * a.old_stride;
 
     double s[6] = {0., 0., 0., 0., 0., 0.};
+    const bool old_sorted = is_ascending(lold, len_old, lane), new_sorted = is_ascending(lnew, len_new, lane);
     for (int32_t base = 0; base < len_new; base += 32) {  // members of L_new that are not in L_old: +
         const int32_t e = base + lane;
         const int32_t j = (e < len_new) ? lnew[e] : -2;
-        if (!in_list(j, lold, len_old, lane) && j >= 0) signed_pair(pi, a.gather, a.n, i, j, 1.0, s);
+        const bool common = old_sorted ? in_sorted_list(j, lold, len_old) : in_list(j, lold, len_old, lane);
+        if (!common && j >= 0) signed_pair(pi, a.gather, a.n, i, j, 1.0, s);
     }
     for (int32_t base = 0; base < len_old; base += 32) {  // members of L_old that are not in L_new: -
         const int32_t e = base + lane;
         const int32_t j = (e < len_old) ? lold[e] : -2;
-        if (!in_list(j, lnew, len_new, lane) && j >= 0) signed_pair(pi, a.gather, a.n, i, j, -1.0, s);
+        const bool common = new_sorted ? in_sorted_list(j, lnew, len_new) : in_list(j, lnew, len_new, lane);
+        if (!common && j >= 0) signed_pair(pi, a.gather, a.n, i, j, -1.0, s);
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {

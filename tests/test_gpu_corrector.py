@@ -6,7 +6,7 @@ Acceptance:
    list (the plain definition); the GPU adds the list difference to the new-list force.  Its error is that of the
    new-list force (north_star: 1e-6 |acc|, 1e-5 |jerk|) plus that of the fp32 pair terms that do NOT cancel, the
    members of L_new xor L_old, measured against their summed norms as for the irregular force (1e-6).  The common
-   members cancel in fp64.
+   members are never evaluated.
  * d2, d3, dx, dv are linear in (f1, fd1): with e_f = |f1_gpu - f1_or|, e_d = |fd1_gpu - fd1_or| of the row,
    |e d2| <= 6 e_f/h^2 + 4 e_d/h, |e d3| <= 12 e_f/h^3 + 6 e_d/h^2, |e dx| <= 0.15 h^2 e_f + h^3 e_d/30,
    |e dv| <= 0.5 h e_f + h^2 e_d/12 (coefficients of f1, fd1 in the formulas of reading R17), plus fp64 rounding.
@@ -175,4 +175,38 @@ def test_hermite_on_the_device_reproduces_a_quintic(oracle):
     assert np.abs(out["dx"].cpu().numpy() - x_beyond).max() < 1e-13
     assert np.abs(out["dv"].cpu().numpy() - v_beyond).max() < 1e-13
     assert torch.equal(out["f1"].cpu(), torch.from_numpy(f1))
+    ctx.close()
+
+
+def test_unsorted_lists_take_the_general_path(oracle):
+    """nb_regular_force writes ascending lists (binary-search membership); any order must give the same result
+    (shuffle-scan membership): same fp32 terms, fp64 sums in another order."""
+    wl = inputs.make_custom(6000, 900, 40, 128, predict=lambda s: oracle.predict_state(s)[0])
+    s = wl.state
+    rs_old = wl.r_s * np.random.default_rng(9).uniform(0.8, 1.2, size=wl.n_i)
+    ctx = binding.Context(s.n, wl.n_i, 128)
+    ctx.set_state(s)
+    dev = ctx.workspace.device
+    i_idx = _t(wl.i_idx, dev, np.int32)
+    old = ctx.nb_regular_force(i_idx, _t(rs_old, dev), s.t)
+    new = ctx.nb_regular_force(i_idx, _t(wl.r_s, dev), s.t)
+    dt, fr0, frd0, n_p = _step_inputs(wl.n_i, 40, 1.0, 5)
+    common = (i_idx, _t(dt, dev), _t(fr0, dev), _t(frd0, dev), new["acc"], new["jerk"])
+    ref = ctx.nb_regular_correct(*common, new["nbr_count"], new["nbr_list"], old["nbr_count"], old["nbr_list"], s.t)
+    rng = np.random.default_rng(10)
+    shuffled = {}
+    for name, d in (("old", old), ("new", new)):
+        lst, cnt = d["nbr_list"].cpu().numpy().copy(), d["nbr_count"].cpu().numpy()
+        assert all(np.all(np.diff(lst[q, :cnt[q]]) > 0) for q in range(wl.n_i))     # ascending as written
+        for q in range(wl.n_i):
+            lst[q, :cnt[q]] = rng.permutation(lst[q, :cnt[q]])
+        shuffled[name] = _t(lst, dev)
+    for new_l, old_l in ((shuffled["new"], shuffled["old"]), (new["nbr_list"], shuffled["old"]),
+                         (shuffled["new"], old["nbr_list"])):
+        got = ctx.nb_regular_correct(*common, new["nbr_count"], new_l, old["nbr_count"], old_l, s.t)
+        torch.cuda.synchronize()
+        for key in ("f1", "fd1"):
+            d = (got[key] - ref[key]).abs().max().item()
+            assert d <= 1e-13 * ref[key].abs().max().item(), (key, d)
+    assert (ref["f1"] - new["acc"]).abs().max().item() > 1e-6     # lists differ, the correction is not zero
     ctx.close()
