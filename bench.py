@@ -187,7 +187,15 @@ def run_sweep(args):
     state_dev = ctx.set_state(s)
     dev = ctx.workspace.device
     rows = []
-    for n_i in inputs.CONFIG3_BLOCKS:
+    blocks = inputs.CONFIG3_BLOCKS
+    if args.sweep_large:       # the same sweep on the N = 2^20 state of config 5 (predict-all costs 38 us there)
+        full = inputs.make_workload(5)
+        s = full.state
+        ctx.close()
+        ctx = binding.Context(s.n, full.n_i, full.cap)
+        state_dev = ctx.set_state(s)
+        blocks = [b for b in inputs.CONFIG3_BLOCKS if b <= 16384]
+    for n_i in blocks:
         i_idx = torch.from_numpy(full.i_idx[:n_i].copy()).to(dev)
         r_s = torch.from_numpy(full.r_s[:n_i].copy()).to(dev)
         out = ctx.alloc_outputs(n_i)
@@ -227,8 +235,32 @@ def run_sweep(args):
         us_graph = gv[0].elapsed_time(gv[1]) / reps * 1e3
         del graph
         info = ctx.nb_last_launch_info()
+        # irregular force of the same block over the lists just made: predict-all + gather (PRED_ALL) against the
+        # prediction fused into the gather (PRED_ACT), each with a fresh prediction per call
+        irr = None
+        iv = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        for _ in range(3):
+            irr = ctx.nb_irregular_force(i_idx, out["nbr_count"], out["nbr_list"], s.t, out=irr)
+            ctx.nb_irregular_force_act(i_idx, out["nbr_count"], out["nbr_list"], s.t, out=irr)
+        torch.cuda.synchronize()
+        iv[0].record()
+        ctx.nb_set_option("irr_pred", 1)
+        for _ in range(reps):
+            ctx.nb_set_j(*state_dev)
+            ctx.nb_irregular_force(i_idx, out["nbr_count"], out["nbr_list"], s.t, out=irr)
+        ctx.nb_set_option("irr_pred", 0)
+        iv[1].record()
+        torch.cuda.synchronize()
+        iv[2].record()
+        for _ in range(reps):
+            ctx.nb_set_j(*state_dev)
+            ctx.nb_irregular_force_act(i_idx, out["nbr_count"], out["nbr_list"], s.t, out=irr)
+        iv[3].record()
+        torch.cuda.synchronize()
         rows.append({"n_i": n_i, "us_per_call": us, "gpairs": n_i * s.n / us / 1e3, "us_fused": us_fused, "us_fused_graph": us_graph,
-                     "rows_per_cta": info["rows_per_cta"], "j_chunks": info["j_chunks"], "ctas": info["ctas"]})
+                     "rows_per_cta": info["rows_per_cta"], "j_chunks": info["j_chunks"], "ctas": info["ctas"],
+                     "us_irr_pred_all": iv[0].elapsed_time(iv[1]) / reps * 1e3,
+                     "us_irr_pred_act": iv[2].elapsed_time(iv[3]) / reps * 1e3})
     print(json.dumps({"metric": METRIC, "unit": UNIT, "config": {"workload": "BASELINE.json configs[2] block sweep",
                                                                  "n": s.n, "timing": "back-to-back calls between two events"},
                       "sweep": rows}))
@@ -442,6 +474,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--n-i", type=int, default=None, help="active-block size (configs 1, 3, 5 only)")
+    ap.add_argument("--sweep-large", action="store_true", help="with --sweep: blocks 32 ... 16384 of the config 5 state")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-irregular", action="store_true")

@@ -117,8 +117,9 @@ int nb_regular_force_ex(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const do
 /* Step (iv), eq. (7), (8), PAPER.md:94-98 (the job of the paper's GPUIRR library): the IRREGULAR
  * force and its time derivative of n_i active particles, summed over the members of their neighbour lists,
  *   acc = sum_{j in L} m_j R_ij / r^3,   jerk = sum_{j in L} m_j [V_ij / r^3 - 3 (R_ij.V_ij) R_ij / r^5],
- * on the state predicted to time t (if t differs from the last prediction, nb_predict_j(t) runs first on the same
- * stream: all particles are predicted, the paper's PRED_ALL mode).  Coordinate differences are two-float
+ * on the state predicted to time t (if t differs from the last prediction, either nb_predict_j(t) runs first on the
+ * same stream -- all particles are predicted, the paper's PRED_ALL mode -- or, for a small block, the gathered
+ * particles are predicted on the spot, PRED_ACT: see nb_irregular_force_act and option "irr_pred").  Coordinate differences are two-float
  * (PAPER.md:138), pair arithmetic fp32, the sum fp64 over 32 fp32 lane sums.
  *   i_idx:       dev int32[n_i]               0-based particle indices
  *   nbr_count:   dev int32[n_i]               list lengths; min(count, list_stride) entries are used
@@ -129,6 +130,17 @@ int nb_regular_force_ex(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const do
 int nb_irregular_force(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const int32_t* nbr_count,
                        const int32_t* nbr_list, int32_t list_stride, double t, double* acc, double* jerk,
                        void* stream);
+
+/* The same sums with the prediction FUSED into the gather: the paper's PRED_ACT mode ("When N_act,I is
+ * small, predicting all the N particles is not efficient.  Thus, at some point (cf. NPACT ...) we switch to predict
+ * only the necessary particles in this block-step").  Every gathered particle is predicted on the spot from the
+ * fp64 state registered with nb_set_j (the predictor's formula, split and roundings, so both modes evaluate the same
+ * fp32 records and return the same bits); no prediction pass runs and the context's predicted records are neither
+ * used nor changed.  One kernel.  Costs 112 B instead of 48 B per gathered particle: for small blocks only (turn-
+ * around measured in DESIGN.md section 5.6).  Arguments and return codes as nb_irregular_force. */
+int nb_irregular_force_act(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const int32_t* nbr_count,
+                           const int32_t* nbr_list, int32_t list_stride, double t, double* acc, double* jerk,
+                           void* stream);
 
 /* Step (vii), PAPER.md:110 ("Execute the regular corrector.  Since the neighbour list L_i has been updated, the
  * force polynomials should be corrected to reflect the difference between the old and new list"), and the
@@ -196,6 +208,9 @@ int nb_regular_force_host(nb_ctx* ctx, int64_t n, const double* x0, const double
  *   "i_block"   force the rows per CTA: 32, 64, 128, 256 or 512 (0 = automatic)
  *   "order_rows" 1 (default): large enough blocks are processed in Morton order of the predicted positions
  *               (results go to the caller's rows all the same); 0: always in the order given; 2: always ordered
+ *   "irr_pred"  how nb_irregular_force gets its predicted particles when the context holds no prediction at t:
+ *               0 (default): rows <= n / 96 predict what they gather (as nb_irregular_force_act), larger blocks
+ *               predict all n first; 1: always predict all; 2: always fused.  Results are identical bit for bit
  * Returns NB_E_INVAL for an unknown key or value. */
 int nb_set_option(nb_ctx* ctx, const char* key, int64_t value);
 

@@ -50,6 +50,7 @@ def load(build_if_missing: bool = True):
     lib.nb_regular_force.argtypes = [vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp, vp]
     lib.nb_regular_force_ex.argtypes = [vp, i32, vp, vp, vp, dbl, vp, vp, vp, vp, vp, vp, vp]
     lib.nb_irregular_force.argtypes = [vp, i32, vp, vp, vp, i32, dbl, vp, vp, vp]
+    lib.nb_irregular_force_act.argtypes = [vp, i32, vp, vp, vp, i32, dbl, vp, vp, vp]
     lib.nb_regular_correct.argtypes = [vp, i32, ctypes.POINTER(CorrectorIO), dbl, vp]
     lib.nb_regular_force_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp]
     lib.nb_set_option.argtypes = [vp, ctypes.c_char_p, i64]
@@ -192,18 +193,23 @@ class Context:
         return out
 
     # -- nb_irregular_force: eq. (7), (8) over given neighbour lists
-    def nb_irregular_force(self, i_idx, nbr_count, nbr_list, t: float, out=None, stream=None):
+    def nb_irregular_force(self, i_idx, nbr_count, nbr_list, t: float, out=None, stream=None, act: bool = False):
         n_i = int(i_idx.shape[0])
         dev = self.workspace.device
         if out is None:
             out = dict(acc=torch.empty((n_i, 3), dtype=torch.float64, device=dev),
                        jerk=torch.empty((n_i, 3), dtype=torch.float64, device=dev))
         stride = int(nbr_list.shape[1]) if nbr_list.dim() == 2 else 1
-        _check(self.lib.nb_irregular_force(
+        fn = self.lib.nb_irregular_force_act if act else self.lib.nb_irregular_force
+        _check(fn(
             self._h, n_i, _dev(i_idx, torch.int32, "i_idx"), _dev(nbr_count, torch.int32, "nbr_count"),
             _dev(nbr_list, torch.int32, "nbr_list"), stride, float(t),
             _dev(out["acc"], torch.float64, "acc"), _dev(out["jerk"], torch.float64, "jerk"), _stream_ptr(stream)))
         return out
+
+    def nb_irregular_force_act(self, i_idx, nbr_count, nbr_list, t: float, out=None, stream=None):
+        """Prediction fused into the gather (PRED_ACT)."""
+        return self.nb_irregular_force(i_idx, nbr_count, nbr_list, t, out=out, stream=stream, act=True)
 
     # -- nb_regular_correct: step (vii) and eq. (1)
     def nb_regular_correct(self, i_idx, dt_r, fr0, frd0, acc, jerk, nbr_count, nbr_list, old_count, old_list, t: float,

@@ -17,7 +17,14 @@
 
 namespace nbreg {
 
+// The registered fp64 state (nb_set_j) and the time to predict to: what the fused-prediction variant gathers from.
+struct RawState {
+    const double *x0, *v0, *a0, *j0, *m, *t0;
+    double t;
+};
+
 struct IrregularArgs {
+    RawState raw;              // irregular_kernel<true> only
     const float4* gather;      // particle-major predicted records, 3 float4 per particle (nbreg_common.cuh)
     int32_t n;                 // j-particles (entries outside [0, n) are ignored)
     int32_t n_i;
@@ -49,12 +56,37 @@ __device__ __forceinline__ PredRecord load_record(const float4* gather, int32_t 
     return r;
 }
 
+// The paper's PRED_ACT mode ("When N_act,I is small, predicting all the N particles is not efficient.
+// Thus ... we switch to predict only the necessary particles in this block-step"): gather a particle's fp64 state
+// (14 scalar loads, 112 B) and predict it on the spot -- the Horner form, the two-float split and the roundings of
+// predict.cuh, so that both modes feed the pair arithmetic the same record.  No prediction pass, no dependence on
+// the context's predicted records: one launch for a small irregular block.
+__device__ __forceinline__ PredRecord predict_record(const RawState& s, int32_t j) {
+    const double dt = s.t - __ldg(s.t0 + j);
+    float h[3], l[3], w[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double x = __ldg(s.x0 + 3 * (size_t)j + c), v = __ldg(s.v0 + 3 * (size_t)j + c);
+        const double acc = __ldg(s.a0 + 3 * (size_t)j + c), jrk = __ldg(s.j0 + 3 * (size_t)j + c);
+        const double xp = x + dt * (v + dt * (0.5 * acc + dt * ((1.0 / 6.0) * jrk)));
+        const double vp = v + dt * (acc + dt * (0.5 * jrk));
+        h[c] = __double2float_rn(xp);
+        l[c] = __double2float_rn(xp - (double)h[c]);
+        w[c] = __double2float_rn(vp);
+    }
+    PredRecord r;
+    r.xh = h[0]; r.yh = h[1]; r.zh = h[2]; r.m = __double2float_rn(__ldg(s.m + j));
+    r.xl = l[0]; r.yl = l[1]; r.zl = l[2]; r.vx = w[0]; r.vy = w[1]; r.vz = w[2];
+    return r;
+}
+
+template <bool ACT>
 __global__ void __launch_bounds__(kIrrWarps * 32) irregular_kernel(IrregularArgs a) {
     const int lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * kIrrWarps + (threadIdx.x >> 5);
     if (row >= a.n_i) return;  // warp-uniform
     const int32_t i = a.i_idx[row];
-    const PredRecord pi = load_record(a.gather, i);
+    const PredRecord pi = ACT ? predict_record(a.raw, i) : load_record(a.gather, i);
     const int32_t len = min(a.nbr_count[row], a.list_stride);
     const int32_t* list = a.nbr_list + (size_t)row * a.list_stride;
 
@@ -62,7 +94,7 @@ __global__ void __launch_bounds__(kIrrWarps * 32) irregular_kernel(IrregularArgs
     for (int32_t e = lane; e < len; e += 32) {
         const int32_t j = list[e];
         if (j == i || j < 0 || j >= a.n) continue;
-        const PredRecord pj = load_record(a.gather, j);
+        const PredRecord pj = ACT ? predict_record(a.raw, j) : load_record(a.gather, j);
         // two-float differences: (xh_j - xh_i) + (xl_j - xl_i)
         const float dx = (pj.xh - pi.xh) + (pj.xl - pi.xl);
         const float dy = (pj.yh - pi.yh) + (pj.yl - pi.yl);

@@ -100,3 +100,45 @@ def test_lists_with_self_garbage_and_empty_rows(oracle):
     assert (np.linalg.norm(a_g - a_o, axis=1)[ok] / sa[ok]).max() <= TOL_TERMS
     assert (np.linalg.norm(j_g - j_o, axis=1)[ok] / sj[ok]).max() <= TOL_TERMS
     ctx.close()
+
+
+def test_fused_prediction_mode_returns_the_same_bits(oracle):
+    """nb_irregular_force_act (the paper's PRED_ACT) predicts each gathered particle on the spot with
+    the predictor's arithmetic: same fp32 records, same sums, bit for bit; it neither needs nor disturbs the
+    context's predicted records."""
+    wl = inputs.make_workload(2, predict=lambda s: oracle.predict_state(s)[0])
+    s = wl.state
+    ctx = binding.Context(s.n, wl.n_i, wl.cap)
+    state_dev = ctx.set_state(s)
+    dev = ctx.workspace.device
+    i_idx = torch.from_numpy(np.ascontiguousarray(wl.i_idx, dtype=np.int32)).to(dev)
+    r_s = torch.from_numpy(np.ascontiguousarray(wl.r_s)).to(dev)
+    reg = ctx.nb_regular_force(i_idx, r_s, s.t)
+    ref = ctx.nb_irregular_force(i_idx, reg["nbr_count"], reg["nbr_list"], s.t)
+    ctx.nb_set_j(*state_dev)                    # no prediction in the context any more
+    act = ctx.nb_irregular_force_act(i_idx, reg["nbr_count"], reg["nbr_list"], s.t)
+    torch.cuda.synchronize()
+    assert torch.equal(act["acc"], ref["acc"]) and torch.equal(act["jerk"], ref["jerk"])
+    # against the oracle, at another time than the context's last prediction, which must survive the call
+    ctx.nb_predict_j(s.t)
+    t2 = s.t + 2.0 ** -7
+    act2 = ctx.nb_irregular_force_act(i_idx, reg["nbr_count"], reg["nbr_list"], t2)
+    again = ctx.nb_irregular_force(i_idx, reg["nbr_count"], reg["nbr_list"], s.t)   # no re-prediction needed
+    torch.cuda.synchronize()
+    assert torch.equal(again["acc"], ref["acc"])
+    # the automatic switch of nb_irregular_force: a small block without a prediction at t runs fused (one launch,
+    # the context's prediction at s.t stays), "irr_pred" = 1 forces the predict-all mode; same bits either way
+    sub = slice(0, 64)
+    auto = ctx.nb_irregular_force(i_idx[sub], reg["nbr_count"][sub], reg["nbr_list"][sub], t2)
+    still = ctx.nb_irregular_force(i_idx, reg["nbr_count"], reg["nbr_list"], s.t)
+    ctx.nb_set_option("irr_pred", 1)
+    forced = ctx.nb_irregular_force(i_idx[sub], reg["nbr_count"][sub], reg["nbr_list"][sub], t2)
+    ctx.nb_set_option("irr_pred", 0)
+    torch.cuda.synchronize()
+    assert torch.equal(auto["acc"], act2["acc"][sub]) and torch.equal(forced["jerk"], act2["jerk"][sub])
+    assert torch.equal(still["acc"], ref["acc"])
+    xp2, vp2 = oracle.predict(s.x0, s.v0, s.a0, s.j0, s.t0, t2)
+    out = dict(nbr_count=reg["nbr_count"].cpu().numpy(), nbr_list=reg["nbr_list"].cpu().numpy(),
+               acc_irr=act2["acc"].cpu().numpy(), jerk_irr=act2["jerk"].cpu().numpy())
+    print(_check_irregular(oracle, xp2, vp2, s.m, wl.i_idx, out, wl.cap))
+    ctx.close()
