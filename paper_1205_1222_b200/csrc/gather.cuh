@@ -134,12 +134,12 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
 
 // The same job with one BLOCK per row, for rows split into many chunks (small active blocks: hundreds of chunks per
 // row and few rows, so a warp per row would leave the machine empty and walk the chunks serially).
-//   Sums: the 128 threads stride over the chunks, xor-shuffle tree per warp, then the four warp sums are added in
+//   Sums: the 512 threads stride over the chunks, xor-shuffle tree per warp, then the 16 warp sums are added in
 //   warp order: fixed order, deterministic.
 //   List: ascending j is plain ascending VALUE, and a row holds few entries compared with its chunks, so each
 //   thread ranks one entry against the staged row (rank = number of smaller entries; entries are distinct) and
-//   stores it at its rank: O(count^2 / 128) instead of O(chunks).
-constexpr int kWideThreads = 128;
+//   stores it at its rank: O(count^2 / 512) instead of O(chunks).
+constexpr int kWideThreads = 512;  // 2048 chunks = 4 dependent rounds of loads per thread (128 threads: 16 rounds, 14 us)
 
 __global__ void __launch_bounds__(kWideThreads) reduce_gather_wide_kernel(GatherArgs a) {
     extern __shared__ int32_t stage[];  // cap entries
@@ -174,7 +174,9 @@ __global__ void __launch_bounds__(kWideThreads) reduce_gather_wide_kernel(Gather
     for (int32_t e = tid; e < stored; e += kWideThreads) stage[e] = out[e];
     __syncthreads();
     if (tid < 7 && tid < n_sums) {
-        const double v = ((warp_sum[0][tid] + warp_sum[1][tid]) + warp_sum[2][tid]) + warp_sum[3][tid];
+        double v = warp_sum[0][tid];
+#pragma unroll
+        for (int w = 1; w < kWideThreads / 32; ++w) v += warp_sum[w][tid];  // fixed order
         if (tid < 3) a.acc[row * 3 + tid] = v;
         else if (tid < 6) a.jerk[row * 3 + tid - 3] = v;
         else a.pot[row] = v;
