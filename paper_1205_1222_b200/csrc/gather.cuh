@@ -134,16 +134,22 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
 
 // The same job with one BLOCK per row, for rows split into many chunks (small active blocks: hundreds of chunks per
 // row and few rows, so a warp per row would leave the machine empty and walk the chunks serially).
-//   Sums: the 512 threads stride over the chunks, xor-shuffle tree per warp, then the 16 warp sums are added in
+//   Sums: the threads stride over the chunks, xor-shuffle tree per warp, then the warp sums are added in
 //   warp order: fixed order, deterministic.
 //   List: ascending j is plain ascending VALUE, and a row holds few entries compared with its chunks, so each
 //   thread ranks one entry against the staged row (rank = number of smaller entries; entries are distinct) and
-//   stores it at its rank: O(count^2 / 512) instead of O(chunks).
-constexpr int kWideThreads = 512;  // 2048 chunks = 4 dependent rounds of loads per thread (128 threads: 16 rounds, 14 us)
+//   stores it at its rank: O(count^2 / threads) instead of O(chunks).
+// Threads per row: 128, or 512 when there are few rows (at most kWideFewRows: then the blocks do not fill the SMs
+// anyway, and 2048 chunks are 4 dependent rounds of loads per thread instead of 16).  With many rows 512-thread
+// blocks lose: fewer resident blocks, most threads idle in the rank sort (measured: N_i = 4096, 321 -> 340 us).
+constexpr int kWideThreads = 128;
+constexpr int kWideThreadsFew = 512;
+constexpr int64_t kWideFewRows = 296;
 
-__global__ void __launch_bounds__(kWideThreads) reduce_gather_wide_kernel(GatherArgs a) {
+__global__ void __launch_bounds__(kWideThreadsFew) reduce_gather_wide_kernel(GatherArgs a) {
     extern __shared__ int32_t stage[];  // cap entries
-    __shared__ double warp_sum[kWideThreads / 32][7];
+    __shared__ double warp_sum[kWideThreadsFew / 32][7];
+    const int n_threads = blockDim.x;  // kWideThreads or kWideThreadsFew
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t prow = blockIdx.x;
     const int64_t lrow = a.row0 + prow;  // grid = split rows exactly
@@ -153,7 +159,7 @@ __global__ void __launch_bounds__(kWideThreads) reduce_gather_wide_kernel(Gather
 
     double s[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     const int n_sums = a.pot ? 7 : 6;
-    for (int c = tid; c < S; c += kWideThreads) {
+    for (int c = tid; c < S; c += n_threads) {
         const double* ps = a.part_sum + (rbase + c) * n_sums;
 #pragma unroll
         for (int k = 0; k < 7; ++k)
@@ -171,17 +177,16 @@ __global__ void __launch_bounds__(kWideThreads) reduce_gather_wide_kernel(Gather
     const int32_t cnt = a.slot_count[prow];  // true count, may exceed cap
     const int32_t stored = min(cnt, a.cap);
     int32_t* out = a.nbr_list + (size_t)row * a.cap;
-    for (int32_t e = tid; e < stored; e += kWideThreads) stage[e] = out[e];
+    for (int32_t e = tid; e < stored; e += n_threads) stage[e] = out[e];
     __syncthreads();
     if (tid < 7 && tid < n_sums) {
         double v = warp_sum[0][tid];
-#pragma unroll
-        for (int w = 1; w < kWideThreads / 32; ++w) v += warp_sum[w][tid];  // fixed order
+        for (int w = 1; w < n_threads / 32; ++w) v += warp_sum[w][tid];  // fixed order
         if (tid < 3) a.acc[row * 3 + tid] = v;
         else if (tid < 6) a.jerk[row * 3 + tid - 3] = v;
         else a.pot[row] = v;
     }
-    for (int32_t e = tid; e < stored; e += kWideThreads) {
+    for (int32_t e = tid; e < stored; e += n_threads) {
         const int32_t v = stage[e];
         int32_t rank = 0;
         for (int32_t k = 0; k < stored; ++k) rank += stage[k] < v;  // broadcast reads

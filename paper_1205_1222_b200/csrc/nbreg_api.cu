@@ -590,7 +590,8 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         const int64_t split_rows = has_split ? n_i - row0 : 0;
         const unsigned blocks = (unsigned)std::max<int64_t>(1, (split_rows + kGatherWarps - 1) / kGatherWarps);
         if (has_split && p.n_chunks > kWideGatherChunks && split_rows <= kWideGatherRows) {  // few rows, many chunks
-            reduce_gather_wide_kernel<<<(unsigned)split_rows, kWideThreads, (size_t)c->cap * sizeof(int32_t), st>>>(ga);
+            reduce_gather_wide_kernel<<<(unsigned)split_rows, split_rows <= kWideFewRows ? kWideThreadsFew : kWideThreads,
+                                        (size_t)c->cap * sizeof(int32_t), st>>>(ga);
         } else {
             const size_t stage = (size_t)kGatherWarps * (c->cap + p.n_chunks) * sizeof(int32_t);
             reduce_gather_kernel<<<blocks, kGatherWarps * 32, stage, st>>>(ga);

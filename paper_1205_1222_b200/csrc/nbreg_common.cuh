@@ -25,7 +25,7 @@ constexpr int kGatherQuads = 3;        // float4 per particle of the particle-ma
 constexpr int kBytesPerJ = 40;         // packed bytes per j-particle
 constexpr int kJPad = 256;             // packed array length is a multiple of this (largest j-tile)
 constexpr float kFarAway = 1.0e18f;    // coordinate of the massless padding particles
-constexpr int kMaxChunks = 2048;       // most j-chunks a row block is split into
+constexpr int kMaxChunks = 4096;       // most j-chunks a row block is split into
 constexpr int kMaxNbrCap = 8192;       // nbr_cap limit: the gather kernel stages 4 rows of cap entries in shared memory
 
 __host__ __device__ inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
