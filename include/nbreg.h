@@ -86,7 +86,7 @@ int nb_get_predicted(nb_ctx* ctx, double* xp, double* vp, void* stream);
  *   neighbour  iff |R_ij|^2 <  r_s^2 : j goes to the list, nothing is summed;
  *   otherwise                        : acc += m_j R_ij / r^3,  jerk += m_j [V_ij / r^3 - 3 (R_ij.V_ij) R_ij / r^5].
  * If t differs from the time of the last prediction, nb_predict_j(t) runs first on the same stream (the fused
- * call).  Differences are formed from the double-single positions, pair arithmetic is fp32 with rsqrt, partial
+ * call), or, for a small block, the prediction runs inside the force kernel (option "fuse_pred").  Differences are formed from the double-single positions, pair arithmetic is fp32 with rsqrt, partial
  * sums are flushed to fp64 every j-tile; outputs are fp64.
  *   n_i:        0 <= n_i <= n_i_max (0 is a no-op that only zeroes n_overflow)
  *   i_idx:      dev int32[n_i]   0-based indices into the j arrays; duplicates allowed
@@ -208,6 +208,10 @@ int nb_regular_force_host(nb_ctx* ctx, int64_t n, const double* x0, const double
  *   "i_block"   force the rows per CTA: 32, 64, 128, 256 or 512 (0 = automatic)
  *   "order_rows" 1 (default): large enough blocks are processed in Morton order of the predicted positions
  *               (results go to the caller's rows all the same); 0: always in the order given; 2: always ordered
+ *   "fuse_pred" 1 (default): a regular-force call that finds no prediction at t, uses the plain criterion without
+ *               potential and fits ONE row block (<= 128 rows) predicts inside the force kernel instead of running
+ *               nb_predict_j first, when n >= 262144 (every j is predicted once, by the CTA that uses it; the context
+ *               then holds no prediction at t); 0: never; 2: also for smaller n.  Results are identical bit for bit
  *   "irr_pred"  how nb_irregular_force gets its predicted particles when the context holds no prediction at t:
  *               0 (default): rows <= n / 96 predict what they gather (as nb_irregular_force_act), larger blocks
  *               predict all n first; 1: always predict all; 2: always fused.  Results are identical bit for bit

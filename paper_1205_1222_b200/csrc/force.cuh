@@ -24,6 +24,7 @@
 //     blocks are all tail.
 #pragma once
 #include "nbreg_common.cuh"
+#include "record.cuh"
 
 namespace nbreg {
 
@@ -36,6 +37,7 @@ namespace nbreg {
 constexpr float kFarFraction2 = NBREG_KAPPA2;
 
 struct ForceArgs {
+    RawState raw;           // PRED: the registered fp64 state and the time to predict to
     const float4* packed;   // packed j-pair records, n_pad / 2 pairs
     int32_t n;              // real j-particles
     int32_t n_tiles;        // number of JT-sized tiles covering n_pad
@@ -254,8 +256,15 @@ __device__ __forceinline__ void append(IState& I, int32_t j, bool nb, int32_t ca
     }
 }
 
-template <int IPT, int WARPS, int JT, int MINB, bool VEL, bool POT>
+// PRED: the predictor fused into the kernel (north_star: "fused with the Hermite predictor of the j-particles").  Used
+// when the whole active block is ONE row block (N_i <= 128), whose j-range is split over the CTAs so that every j is
+// predicted exactly once, by the CTA that uses it: each thread predicts one pair of consecutive j per tile from the
+// registered fp64 state (predict_record: the arithmetic of predict.cuh, the same records bit for bit) and writes its
+// packed record straight into the shared-memory tile -- no prediction pass (38 us at N = 2^20), no packed records in
+// HBM.  The CTAs resident on an SM hide each other's load latency; there is one tile stage and no bulk copy.
+template <int IPT, int WARPS, int JT, int MINB, bool VEL, bool POT, bool PRED = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
+    static_assert(!PRED || (IPT == 1 && JT == 2 * WARPS * 32 && !VEL), "PRED: one j-pair per thread per tile");
     constexpr int kSums = POT ? 7 : 6;  // fp64 running sums per row: acc, jerk (, pot)
     constexpr int kThreads = WARPS * 32;
     constexpr int kRows = kThreads * IPT;
@@ -285,12 +294,12 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
     const int n_t = t_end - t_begin;
     const int64_t tail_row0 = (int64_t)a.main_blocks * kRows;
 
-    if (tid == 0) {
+    if (!PRED && tid == 0) {
         for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
     }
-    __syncthreads();
-    if (tid == 0 && n_t > 0) {  // prologue: first tile in flight while the i-state is gathered
+    if (!PRED) __syncthreads();
+    if (!PRED && tid == 0 && n_t > 0) {  // prologue: first tile in flight while the i-state is gathered
         mbar_arrive_expect_tx(&full[0], kTileBytes);
         bulk_g2s(tiles, a.packed + (size_t)t_begin * kTileQuads, kTileBytes, &full[0]);
     }
@@ -306,11 +315,17 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         const bool live = row < a.n_i;
         const int64_t orow = (live && a.perm) ? a.perm[row] : row;  // the caller's row
         const int32_t i = live ? a.i_idx[orow] : 0;
-        const float* rec = reinterpret_cast<const float*>(a.packed + (size_t)(i >> 1) * kQuadsPerPair);
-        const int h = i & 1;
-        const float xh = rec[0 + h], yh = rec[2 + h], zh = rec[4 + h];
-        const float vx = rec[8 + h], vy = rec[10 + h], vz = rec[12 + h];
-        const float xl = rec[14 + h], yl = rec[16 + h], zl = rec[18 + h];
+        float xh, yh, zh, vx, vy, vz, xl, yl, zl;
+        if (PRED) {
+            const PredRecord ri = predict_record(a.raw, i);
+            xh = ri.xh; yh = ri.yh; zh = ri.zh; vx = ri.vx; vy = ri.vy; vz = ri.vz; xl = ri.xl; yl = ri.yl; zl = ri.zl;
+        } else {
+            const float* rec = reinterpret_cast<const float*>(a.packed + (size_t)(i >> 1) * kQuadsPerPair);
+            const int h = i & 1;
+            xh = rec[0 + h]; yh = rec[2 + h]; zh = rec[4 + h];
+            vx = rec[8 + h]; vy = rec[10 + h]; vz = rec[12 + h];
+            xl = rec[14 + h]; yl = rec[16 + h]; zl = rec[18 + h];
+        }
         I[u].nxh = -xh; I[u].nyh = -yh; I[u].nzh = -zh;
         I[u].nxl = -xl; I[u].nyl = -yl; I[u].nzl = -zl;
         I[u].nvx = -vx; I[u].nvy = -vy; I[u].nvz = -vz;
@@ -341,13 +356,28 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
 
     // ---- S3/S4: stream the j-tiles
     for (int lt = 0; lt < n_t; ++lt) {
-        const int st = lt & 1;
-        if (tid == 0 && lt + 1 < n_t) {  // prefetch the next tile into the other stage (freed by the barrier below)
+        const int st = PRED ? 0 : (lt & 1);
+        if (PRED) {  // predict this thread's j-pair of the tile into shared memory (layout of nbreg_common.cuh)
+            const int32_t j0 = (t_begin + lt) * JT + 2 * tid;
+            PredRecord r0, r1;
+            r0.xh = r0.yh = r0.zh = kFarAway; r0.m = r0.xl = r0.yl = r0.zl = r0.vx = r0.vy = r0.vz = 0.f;
+            r1 = r0;  // padding particles past n: massless, far away, at rest
+            if (j0 < a.n) r0 = predict_record(a.raw, j0);
+            if (j0 + 1 < a.n) r1 = predict_record(a.raw, j0 + 1);
+            float4* o = tiles + tid * kQuadsPerPair;
+            o[0] = make_float4(r0.xh, r1.xh, r0.yh, r1.yh);
+            o[1] = make_float4(r0.zh, r1.zh, r0.m, r1.m);
+            o[2] = make_float4(r0.vx, r1.vx, r0.vy, r1.vy);
+            o[3] = make_float4(r0.vz, r1.vz, r0.xl, r1.xl);
+            o[4] = make_float4(r0.yl, r1.yl, r0.zl, r1.zl);
+            if (WARPS > 1) __syncthreads(); else __syncwarp();
+        }
+        if (!PRED && tid == 0 && lt + 1 < n_t) {  // prefetch the next tile into the other stage (freed by the barrier below)
             mbar_arrive_expect_tx(&full[st ^ 1], kTileBytes);
             bulk_g2s(tiles + (st ^ 1) * kTileQuads, a.packed + (size_t)(t_begin + lt + 1) * kTileQuads, kTileBytes,
                      &full[st ^ 1]);
         }
-        mbar_wait(&full[st], (lt >> 1) & 1);
+        if (!PRED) mbar_wait(&full[st], (lt >> 1) & 1);
         const float4* tp = tiles + st * kTileQuads;
         const int32_t jbase = (t_begin + lt) * JT;
         if (VEL) {  // far threshold of this tile: its fastest particle cannot bring a far pair within r_s during dtr

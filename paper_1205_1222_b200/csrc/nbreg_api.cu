@@ -141,7 +141,7 @@ struct nb_ctx {
     bool predicted = false;
     double t_pred = 0.0;
     // options
-    int64_t opt_j_split = 0, opt_i_block = 0, opt_order_rows = 1, opt_irr_pred = 0;
+    int64_t opt_j_split = 0, opt_i_block = 0, opt_order_rows = 1, opt_irr_pred = 0, opt_fuse_pred = 1;
     // last launch
     int64_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     // host path: device mirrors owned by the context
@@ -163,6 +163,7 @@ namespace {
 // ragged end, which is why several waves of short CTAs beat one wave of long ones.
 // rows split into more than kWideGatherChunks chunks are gathered by a block each, if there are few enough of them
 // that a warp per row would leave SMs idle
+constexpr int64_t kFusePredMinN = 262144;  // smallest n for which a one-row-block call predicts inside the force kernel
 constexpr int kOrderMinRows = 256;  // smaller active blocks are processed in the order given
 constexpr int kWideGatherChunks = 64;
 constexpr int64_t kWideGatherRows = 4096;
@@ -285,6 +286,30 @@ int launch_force(const Plan& p, const ForceArgs& fa, cudaStream_t st) {
     force_kernel<IPT, WARPS, JT, MINB, VEL, POT><<<p.grid, WARPS * 32, smem, st>>>(fa);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
+}
+
+// The fused-prediction variant (force.cuh, PRED): plain criterion, no potential, shapes of 128 / 64 / 32 rows.
+int launch_force_pred(int shape, const Plan& p, const ForceArgs& fa, cudaStream_t st) {
+#define NB_PRED(WARPS, JT, MINB)                                                                    \
+    {                                                                                               \
+        auto kern = force_kernel<1, WARPS, JT, MINB, false, false, true>;                           \
+        const size_t smem = force_smem_bytes(1, WARPS, JT, false);                                  \
+        static bool attr_set = false;                                                               \
+        if (!attr_set) {                                                                            \
+            NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+            attr_set = true;                                                                        \
+        }                                                                                           \
+        kern<<<p.grid, WARPS * 32, smem, st>>>(fa);                                                 \
+        NB_CUDA(cudaGetLastError());                                                                \
+        return NB_OK;                                                                               \
+    }
+    switch (shape) {
+        case 1: NB_PRED(4, 256, NBREG_WARPS_SMALL / 4)
+        case 2: NB_PRED(2, 128, NBREG_WARPS_SMALL / 2)
+        case 3: NB_PRED(1, 64, NBREG_WARPS_SMALL)
+        default: return NB_E_INVAL;
+    }
+#undef NB_PRED
 }
 
 // one switch for both: keeps the template arguments of query and launch in one place.  variant: bit 0 = velocity
@@ -498,7 +523,24 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     NB_CUDA(cudaSetDevice(c->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int launches = 0;
-    if (!c->predicted || c->t_pred != t) {  // the fused call: S1 first, same stream
+    const bool stale = !c->predicted || c->t_pred != t;
+    // A block of one row block (<= 128 rows) with the plain criterion predicts inside the force kernel: its j-range is
+    // split over the CTAs, so every j is predicted once, by the CTA that uses it (force.cuh, PRED).
+    bool fuse_pred = false;
+    // It pays when the prediction pass is long: measured at N = 2^20, N_i = 32: 94.8 -> 73.4 us per call (the pass costs
+    // 38 us, reading the fp64 state in the force kernel 19 us); at N = 65536 the pass costs 5 us and the fused kernel's
+    // exposed load latency more (29.4 -> 32.1 us), hence the size limit ("fuse_pred" = 2 lifts it).
+    const bool big = c->n >= kFusePredMinN || c->opt_fuse_pred == 2;
+    if (stale && n_i > 0 && !dtr && !pot && c->opt_fuse_pred && big && c->opt_order_rows != 2) {
+        Machine m0{};
+        m0.n = c->n;
+        m0.row_chunk_limit = c->lay.row_chunk_limit;
+        m0.num_sms = c->num_sms;
+        for (int k = 0; k < kNumShapes; ++k) m0.ctas_per_sm[k] = c->ctas_per_sm[0][k];
+        const Plan p0 = make_plan(&m0, n_i, c->opt_i_block, c->opt_j_split);
+        fuse_pred = p0.n_blocks == 1 && p0.shape >= 1 && p0.shape <= 3;
+    }
+    if (stale && !fuse_pred) {  // the fused call: S1 first, same stream
         int rc = nb_predict_j(c, t, stream);
         if (rc != NB_OK) return rc;
         ++launches;
@@ -516,6 +558,7 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     for (int k = 0; k < kNumShapes; ++k) mach.ctas_per_sm[k] = c->ctas_per_sm[variant][k];
     const Plan p = make_plan(&mach, n_i, c->opt_i_block, c->opt_j_split);
     ForceArgs fa{};
+    fa.raw = RawState{c->x0, c->v0, c->a0, c->j0, c->m, c->t0, t};
     fa.packed = reinterpret_cast<const float4*>(c->ws + c->lay.packed_off);
     fa.n = (int32_t)c->n;
     fa.n_tiles = p.n_tiles;
@@ -576,7 +619,7 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     }
     fa.slot_count = reinterpret_cast<int32_t*>(c->ws + c->lay.slot_off);
     fa.overflow_ws = ctl;
-    int rc = force_dispatch(variant, p.shape, nullptr, &p, &fa, st);
+    int rc = fuse_pred ? launch_force_pred(p.shape, p, fa, st) : force_dispatch(variant, p.shape, nullptr, &p, &fa, st);
     if (rc != NB_OK) return rc;
     ++launches;
     {  // S5 + n_overflow: always launched, with no rows when nothing was split
@@ -795,6 +838,11 @@ int nb_set_option(nb_ctx* c, const char* key, int64_t value) {
     if (!strcmp(key, "order_rows")) {
         if (value > 2) return NB_E_INVAL;
         c->opt_order_rows = value;
+        return NB_OK;
+    }
+    if (!strcmp(key, "fuse_pred")) {
+        if (value > 2) return NB_E_INVAL;
+        c->opt_fuse_pred = value;
         return NB_OK;
     }
     if (!strcmp(key, "irr_pred")) {

@@ -317,3 +317,39 @@ def test_row_ordering_paths(oracle, n_i):
     xp, vp = oracle.predict_state(wl.state)
     parity.compare(oracle, xp, vp, wl.state.m, wl.i_idx, wl.r_s, wl.cap, g, dtr=dtr, check_pot=True)
     parity.check_overflow_flag(g, wl.cap)
+
+
+@pytest.mark.parametrize("n,n_i", [(5001, 1), (5001, 32), (70001, 64), (70001, 100), (30000, 128), (30000, 129)])
+def test_prediction_fused_into_the_force_kernel_gives_the_same_bits(oracle, n, n_i):
+    """A block of one row block (<= 128 rows) predicts inside force_kernel (PRED variant) instead of running the
+    predictor first: same records, same pair arithmetic, identical outputs; checked against the two-kernel path
+    (option fuse_pred = 0) bit for bit, and against the oracle as usual.  129 rows take the two-kernel path."""
+    wl = inputs.make_custom(n, n_i, 20, 64, seed_sub=7, predict=lambda s: oracle.predict_state(s)[0])
+    s = wl.state
+    ctx = binding.Context(s.n, max(n_i, 1), wl.cap)
+    res = {}
+    for fuse in (2, 0):
+        ctx.nb_set_option("fuse_pred", fuse)      # 2: fuse whenever the block is one row block, whatever n
+        gpu, info = run_gpu(wl, ctx=ctx)          # set_state invalidates the prediction: the call is the fused one
+        res[fuse] = (gpu, info)
+    (g1, i1), (g0, i0) = res[2], res[0]
+    assert i0["launches"] == 3                    # predictor, force, gather
+    one_block = n_i <= i1["rows_per_cta"] <= 128
+    assert i1["launches"] == (2 if one_block else 3)
+    assert one_block or n_i > 32
+    for k in ("acc", "jerk", "nbr_count", "n_overflow"):
+        assert np.array_equal(g1[k], g0[k]), k
+    for q in range(n_i):
+        c = min(g1["nbr_count"][q], wl.cap)
+        assert np.array_equal(g1["nbr_list"][q, :c], g0["nbr_list"][q, :c])
+    xp, vp = oracle.predict_state(s)
+    parity.compare(oracle, xp, vp, s.m, wl.i_idx, wl.r_s, wl.cap, g1)
+    # the context holds no prediction after the fused call: a second call at the same time fuses again, and a
+    # call that needs the predicted records (velocity criterion) predicts first
+    ctx.nb_set_option("fuse_pred", 1)
+    g3, i3 = run_gpu(wl, ctx=ctx)
+    assert i3["launches"] == 3                   # n < 262144: the automatic mode keeps the two-kernel path
+    ctx.nb_set_option("fuse_pred", 2)
+    g2, i2 = run_gpu(wl, ctx=ctx, dtr=np.zeros(n_i))
+    assert i2["launches"] == 3 and np.allclose(g2["acc"], g1["acc"], rtol=1e-5, atol=0)
+    ctx.close()
