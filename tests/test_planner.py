@@ -86,3 +86,15 @@ def test_plan_depends_on_machine_size():
     a = binding.nb_plan(65536, 4096, 148, OCC)
     b = binding.nb_plan(65536, 4096, 16, OCC)
     assert a["ctas"] > b["ctas"] or a["j_chunks"] >= b["j_chunks"]
+
+
+@pytest.mark.parametrize("n", [65536, 1 << 20])
+def test_shapes_much_taller_than_the_block_are_left_out(n):
+    """A CTA shape at least twice as tall as the whole active block would compute rows that do not exist."""
+    for n_i in (1, 7, 32):
+        assert binding.nb_plan(n, n_i, 148, OCC)["rows_per_cta"] == 32
+    for n_i in (33, 64):
+        assert binding.nb_plan(n, n_i, 148, OCC)["rows_per_cta"] <= 64
+    for n_i in (65, 128):
+        assert binding.nb_plan(n, n_i, 148, OCC)["rows_per_cta"] <= 128
+    assert binding.nb_plan(n, 64, 148, OCC, i_block=256)["rows_per_cta"] == 256   # a forced shape is obeyed
