@@ -290,18 +290,12 @@ int launch_force(const Plan& p, const ForceArgs& fa, cudaStream_t st) {
 
 // The fused-prediction variant (force.cuh, PRED): plain criterion, no potential, shapes of 128 / 64 / 32 rows.
 int launch_force_pred(int shape, const Plan& p, const ForceArgs& fa, cudaStream_t st) {
-#define NB_PRED(WARPS, JT, MINB)                                                                    \
-    {                                                                                               \
-        auto kern = force_kernel<1, WARPS, JT, MINB, false, false, true>;                           \
-        const size_t smem = force_smem_bytes(1, WARPS, JT, false);                                  \
-        static bool attr_set = false;                                                               \
-        if (!attr_set) {                                                                            \
-            NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-            attr_set = true;                                                                        \
-        }                                                                                           \
-        kern<<<p.grid, WARPS * 32, smem, st>>>(fa);                                                 \
-        NB_CUDA(cudaGetLastError());                                                                \
-        return NB_OK;                                                                               \
+#define NB_PRED(WARPS, JT, MINB)                                                                      \
+    {                                                                                                 \
+        const size_t smem = force_smem_bytes(1, WARPS, JT, false); /* <= 27 KB: no opt-in needed */   \
+        force_kernel<1, WARPS, JT, MINB, false, false, true><<<p.grid, WARPS * 32, smem, st>>>(fa);   \
+        NB_CUDA(cudaGetLastError());                                                                  \
+        return NB_OK;                                                                                 \
     }
     switch (shape) {
         case 1: NB_PRED(4, 256, NBREG_WARPS_SMALL / 4)
@@ -524,8 +518,8 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int launches = 0;
     const bool stale = !c->predicted || c->t_pred != t;
-    // A block of one row block (<= 128 rows) with the plain criterion predicts inside the force kernel: its j-range is
-    // split over the CTAs, so every j is predicted once, by the CTA that uses it (force.cuh, PRED).
+    // A small block (< 256 rows) with the plain criterion predicts inside the force kernel: its j-range is split over
+    // the CTAs, so every j is predicted by the CTA that uses it (force.cuh, PRED).
     bool fuse_pred = false;
     // It pays when the prediction pass is long: measured at N = 2^20, N_i = 32: 94.8 -> 73.4 us per call (the pass costs
     // 38 us, reading the fp64 state in the force kernel 19 us); at N = 65536 the pass costs 5 us and the fused kernel's
@@ -538,7 +532,10 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         m0.num_sms = c->num_sms;
         for (int k = 0; k < kNumShapes; ++k) m0.ctas_per_sm[k] = c->ctas_per_sm[0][k];
         const Plan p0 = make_plan(&m0, n_i, c->opt_i_block, c->opt_j_split);
-        fuse_pred = p0.n_blocks == 1 && p0.shape >= 1 && p0.shape <= 3;
+        // one row block: every j predicted once.  A few row blocks (N_i < kOrderMinRows = 256, so no row ordering,
+        // which reads predicted records): each predicts its j again, ~3 % more instructions per block and 112 B/j of
+        // HBM reads that hide under the pair arithmetic, against a 38 us pass that nothing overlaps.
+        fuse_pred = n_i < kOrderMinRows && p0.shape >= 1 && p0.shape <= 3;
     }
     if (stale && !fuse_pred) {  // the fused call: S1 first, same stream
         int rc = nb_predict_j(c, t, stream);

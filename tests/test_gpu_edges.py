@@ -319,11 +319,11 @@ def test_row_ordering_paths(oracle, n_i):
     parity.check_overflow_flag(g, wl.cap)
 
 
-@pytest.mark.parametrize("n,n_i", [(5001, 1), (5001, 32), (70001, 64), (70001, 100), (30000, 128), (30000, 129)])
+@pytest.mark.parametrize("n,n_i", [(5001, 1), (5001, 32), (70001, 64), (70001, 100), (30000, 128), (30000, 255), (30000, 256)])
 def test_prediction_fused_into_the_force_kernel_gives_the_same_bits(oracle, n, n_i):
-    """A block of one row block (<= 128 rows) predicts inside force_kernel (PRED variant) instead of running the
-    predictor first: same records, same pair arithmetic, identical outputs; checked against the two-kernel path
-    (option fuse_pred = 0) bit for bit, and against the oracle as usual.  129 rows take the two-kernel path."""
+    """A small block (< 256 rows) predicts inside force_kernel (PRED variant) instead of running the predictor
+    first: same records, same pair arithmetic, identical outputs; checked against the two-kernel path (option
+    fuse_pred = 0) bit for bit, and against the oracle as usual.  256 rows take the two-kernel path."""
     wl = inputs.make_custom(n, n_i, 20, 64, seed_sub=7, predict=lambda s: oracle.predict_state(s)[0])
     s = wl.state
     ctx = binding.Context(s.n, max(n_i, 1), wl.cap)
@@ -334,9 +334,7 @@ def test_prediction_fused_into_the_force_kernel_gives_the_same_bits(oracle, n, n
         res[fuse] = (gpu, info)
     (g1, i1), (g0, i0) = res[2], res[0]
     assert i0["launches"] == 3                    # predictor, force, gather
-    one_block = n_i <= i1["rows_per_cta"] <= 128
-    assert i1["launches"] == (2 if one_block else 3)
-    assert one_block or n_i > 32
+    assert i1["launches"] == (2 if n_i < 256 else 3)
     for k in ("acc", "jerk", "nbr_count", "n_overflow"):
         assert np.array_equal(g1[k], g0[k]), k
     for q in range(n_i):
