@@ -319,7 +319,8 @@ def test_row_ordering_paths(oracle, n_i):
     parity.check_overflow_flag(g, wl.cap)
 
 
-@pytest.mark.parametrize("n,n_i", [(5001, 1), (5001, 32), (70001, 64), (70001, 100), (30000, 128), (30000, 255), (30000, 256)])
+@pytest.mark.parametrize("n,n_i", [(5001, 1), (5001, 32), (70001, 64), (70001, 100), (30000, 128), (30000, 255), (30000, 256),
+                                  (300001, 100)])
 def test_prediction_fused_into_the_force_kernel_gives_the_same_bits(oracle, n, n_i):
     """A small block (< 256 rows) predicts inside force_kernel (PRED variant) instead of running the predictor
     first: same records, same pair arithmetic, identical outputs; checked against the two-kernel path (option
@@ -328,8 +329,9 @@ def test_prediction_fused_into_the_force_kernel_gives_the_same_bits(oracle, n, n
     s = wl.state
     ctx = binding.Context(s.n, max(n_i, 1), wl.cap)
     res = {}
+    big = n >= 262144                             # there the default setting (1) fuses by itself
     for fuse in (2, 0):
-        ctx.nb_set_option("fuse_pred", fuse)      # 2: fuse whenever the block is one row block, whatever n
+        ctx.nb_set_option("fuse_pred", 1 if (fuse and big) else fuse)   # 2: fuse a small block whatever n
         gpu, info = run_gpu(wl, ctx=ctx)          # set_state invalidates the prediction: the call is the fused one
         res[fuse] = (gpu, info)
     (g1, i1), (g0, i0) = res[2], res[0]
@@ -346,7 +348,7 @@ def test_prediction_fused_into_the_force_kernel_gives_the_same_bits(oracle, n, n
     # call that needs the predicted records (velocity criterion) predicts first
     ctx.nb_set_option("fuse_pred", 1)
     g3, i3 = run_gpu(wl, ctx=ctx)
-    assert i3["launches"] == 3                   # n < 262144: the automatic mode keeps the two-kernel path
+    assert i3["launches"] == (2 if big and n_i < 256 else 3)   # n < 262144: automatic mode keeps the two-kernel path
     ctx.nb_set_option("fuse_pred", 2)
     g2, i2 = run_gpu(wl, ctx=ctx, dtr=np.zeros(n_i))
     assert i2["launches"] == 3 and np.allclose(g2["acc"], g1["acc"], rtol=1e-5, atol=0)
