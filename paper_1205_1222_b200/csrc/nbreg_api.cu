@@ -32,6 +32,12 @@ using namespace nbreg;
 #ifndef NBREG_WARPS_SMALL
 #define NBREG_WARPS_SMALL 28
 #endif
+// ... and the fused-prediction variants of those shapes (PRED, force.cuh).  Measured at N = 2^20, N_i = 32 / 64 / 128, us per
+// call: 28 warps (72 registers, 44 B spilled) 73.6 / 105.2 / 189.1; 24 warps (80 registers) 72.1 / 101.2 / 179.2; 20 warps (96
+// registers, no spills) 70.4 / 105.0 / 184.8.
+#ifndef NBREG_WARPS_PRED
+#define NBREG_WARPS_PRED 24
+#endif
 
 namespace {
 
@@ -298,9 +304,9 @@ int launch_force_pred(int shape, const Plan& p, const ForceArgs& fa, cudaStream_
         return NB_OK;                                                                                 \
     }
     switch (shape) {
-        case 1: NB_PRED(4, 256, NBREG_WARPS_SMALL / 4)
-        case 2: NB_PRED(2, 128, NBREG_WARPS_SMALL / 2)
-        case 3: NB_PRED(1, 64, NBREG_WARPS_SMALL)
+        case 1: NB_PRED(4, 256, NBREG_WARPS_PRED / 4)
+        case 2: NB_PRED(2, 128, NBREG_WARPS_PRED / 2)
+        case 3: NB_PRED(1, 64, NBREG_WARPS_PRED)
         default: return NB_E_INVAL;
     }
 #undef NB_PRED
