@@ -209,7 +209,7 @@ int nb_regular_force_host(nb_ctx* ctx, int64_t n, const double* x0, const double
  *   "order_rows" 1 (default): large enough blocks are processed in Morton order of the predicted positions
  *               (results go to the caller's rows all the same); 0: always in the order given; 2: always ordered
  *   "fuse_pred" 1 (default): a regular-force call that finds no prediction at t, uses the plain criterion without
- *               potential and has fewer than 256 rows predicts inside the force kernel instead of running
+ *               potential and has at most 256 rows predicts inside the force kernel instead of running
  *               nb_predict_j first, when n >= 262144 (every j is predicted by the CTA that uses it; the context
  *               then holds no prediction at t); 0: never; 2: also for smaller n.  Results are identical bit for bit
  *   "irr_pred"  how nb_irregular_force gets its predicted particles when the context holds no prediction at t:

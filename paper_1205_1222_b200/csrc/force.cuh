@@ -257,7 +257,7 @@ __device__ __forceinline__ void append(IState& I, int32_t j, bool nb, int32_t ca
 }
 
 // PRED: the predictor fused into the kernel (north_star: "fused with the Hermite predictor of the j-particles").  Used
-// for small active blocks (N_i < 256: one to eight row blocks), whose j-range is split over the CTAs so that every j is
+// for small active blocks (N_i <= 256: one to eight row blocks), whose j-range is split over the CTAs so that every j is
 // predicted by the CTA that uses it (once per row block): each thread predicts one pair of consecutive j per tile from the
 // registered fp64 state (predict_record: the arithmetic of predict.cuh, the same records bit for bit) and writes its
 // packed record straight into the shared-memory tile -- no prediction pass (38 us at N = 2^20), no packed records in

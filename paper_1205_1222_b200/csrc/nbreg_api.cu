@@ -169,6 +169,7 @@ namespace {
 // ragged end, which is why several waves of short CTAs beat one wave of long ones.
 // rows split into more than kWideGatherChunks chunks are gathered by a block each, if there are few enough of them
 // that a warp per row would leave SMs idle
+constexpr int kFusePredMaxRows = 256;     // largest block that predicts inside the force kernel (measured below)
 constexpr int64_t kFusePredMinN = 262144;  // smallest n for which a one-row-block call predicts inside the force kernel
 constexpr int kOrderMinRows = 256;  // smaller active blocks are processed in the order given
 constexpr int kWideGatherChunks = 64;
@@ -524,24 +525,26 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int launches = 0;
     const bool stale = !c->predicted || c->t_pred != t;
-    // A small block (< 256 rows) with the plain criterion predicts inside the force kernel: its j-range is split over
+    // A small block (<= 256 rows) with the plain criterion predicts inside the force kernel: its j-range is split over
     // the CTAs, so every j is predicted by the CTA that uses it (force.cuh, PRED).
     bool fuse_pred = false;
     // It pays when the prediction pass is long: measured at N = 2^20, N_i = 32: 94.8 -> 73.4 us per call (the pass costs
     // 38 us, reading the fp64 state in the force kernel 19 us); at N = 65536 the pass costs 5 us and the fused kernel's
     // exposed load latency more (29.4 -> 32.1 us), hence the size limit ("fuse_pred" = 2 lifts it).
     const bool big = c->n >= kFusePredMinN || c->opt_fuse_pred == 2;
-    if (stale && n_i > 0 && !dtr && !pot && c->opt_fuse_pred && big && c->opt_order_rows != 2) {
+    if (stale && n_i > 0 && !dtr && !pot && c->opt_fuse_pred && big) {
         Machine m0{};
         m0.n = c->n;
         m0.row_chunk_limit = c->lay.row_chunk_limit;
         m0.num_sms = c->num_sms;
         for (int k = 0; k < kNumShapes; ++k) m0.ctas_per_sm[k] = c->ctas_per_sm[0][k];
         const Plan p0 = make_plan(&m0, n_i, c->opt_i_block, c->opt_j_split);
-        // one row block: every j predicted once.  A few row blocks (N_i < kOrderMinRows = 256, so no row ordering,
-        // which reads predicted records): each predicts its j again, ~3 % more instructions per block and 112 B/j of
-        // HBM reads that hide under the pair arithmetic, against a 38 us pass that nothing overlaps.
-        fuse_pred = n_i < kOrderMinRows && p0.shape >= 1 && p0.shape <= 3;
+        // one row block: every j predicted once.  A few row blocks: each predicts its j again, ~3 % more instructions
+        // per block and 112 B/j of HBM reads that hide under the pair arithmetic, against a 38 us pass that nothing
+        // overlaps.  Measured at N = 2^20, fresh prediction per call, pass -> fused: N_i = 128: 201 -> 179 us, 256: 345 ->
+        // 337 us, 512: 606 -> 609 us: it pays up to 256 rows.  The row ordering then predicts its rows' positions itself
+        // (order.cuh, from_raw).
+        fuse_pred = n_i <= kFusePredMaxRows && p0.shape >= 1 && p0.shape <= 3;
     }
     if (stale && !fuse_pred) {  // the fused call: S1 first, same stream
         int rc = nb_predict_j(c, t, stream);
@@ -591,6 +594,8 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         const size_t seg = (size_t)round_up((int64_t)std::max<int64_t>(c->n_i_max, 1) * 4, 256);
         unsigned char* sb = c->ws + c->lay.sort_off;
         OrderArgs oa{};
+        oa.raw = fa.raw;
+        oa.from_raw = fuse_pred;
         oa.gather = reinterpret_cast<const float4*>(c->ws + c->lay.gather_off);
         oa.i_idx = i_idx;
         oa.n_i = n_i;

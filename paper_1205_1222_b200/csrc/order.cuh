@@ -20,6 +20,7 @@
 #include <cub/block/block_radix_sort.cuh>
 
 #include "nbreg_common.cuh"
+#include "record.cuh"
 
 namespace nbreg {
 
@@ -28,6 +29,8 @@ constexpr int kSmallSortRadixBits = 5;  // 24-bit keys in five passes (measured:
 constexpr int kOrderThreads = 256;
 
 struct OrderArgs {
+    RawState raw;           // from_raw: the registered fp64 state and the time to predict to
+    bool from_raw;          // the context holds no prediction (fused-prediction call): predict the rows' positions here
     const float4* gather;   // particle-major predicted records
     const int32_t* i_idx;   // [n_i]
     int32_t n_i;
@@ -61,6 +64,10 @@ __device__ __forceinline__ uint32_t morton_key(float x, float y, float z, const 
     return spread8(qx) | (spread8(qy) << 1) | (spread8(qz) << 2);
 }
 __device__ __forceinline__ float3 row_position(const OrderArgs& a, int32_t q) {
+    if (a.from_raw) {  // the same high words the predictor would have written: the same keys, the same order
+        const PredRecord r = predict_record(a.raw, a.i_idx[q]);
+        return make_float3(r.xh, r.yh, r.zh);
+    }
     const float4 g0 = __ldg(a.gather + (size_t)a.i_idx[q] * kGatherQuads);
     return make_float3(g0.x, g0.y, g0.z);
 }
