@@ -129,8 +129,11 @@ def test_coincident_particles(oracle):
     _full_check(oracle, wl, gpu)
 
 
-def test_host_entry_point_matches_device_entry_point(oracle):
-    wl = _wl(oracle, 3001, 257, 20, 64)
+@pytest.mark.parametrize("n,n_i", [(3001, 257), (270001, 48)])
+def test_host_entry_point_matches_device_entry_point(oracle, n, n_i):
+    """(270001, 48): small block of a large system, the prediction runs inside the force kernel on the context's own
+    device mirrors of the host arrays."""
+    wl = _wl(oracle, n, n_i, 20, 64)
     dev_out, _ = run_gpu(wl)
     s = wl.state
     ctx = binding.Context(s.n, wl.n_i, wl.cap)
