@@ -148,7 +148,8 @@ int nb_irregular_force_act(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const
  * prints no corrector formula; readings R16-R18 of DESIGN.md state what is computed, per row q, i = i_idx[q]:
  *   1. f1, fd1 = acc, jerk + sum_{j in L_new} f_ij - sum_{j in L_old} f_ij: the regular force and its derivative at
  *      t with respect to the OLD list (the one the step was integrated with); f_ij = the pair terms of eq. (7), (8) on
- *      the state predicted to t (predicted first if t differs from the last prediction), fp32 on two-float
+ *      the state predicted to t (if t differs from the last prediction: all particles are predicted first, or, for a
+ *      small block, the gathered ones on the spot -- the switch of nb_irregular_force, option "irr_pred"), fp32 on two-float
  *      differences, summed in fp64;
  *   2. the cubic Hermite polynomial F(tau) through (fr0, frd0) at tau = 0 and (f1, fd1) at tau = dt_r:
  *      d3 = F''' = [12 (fr0 - f1) + 6 dt (frd0 + fd1)] / dt^3,  d2 = F''(dt_r) = [-6 (fr0 - f1) - dt (4 frd0 + 2 fd1)] /

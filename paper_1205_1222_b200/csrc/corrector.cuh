@@ -20,6 +20,7 @@
 namespace nbreg {
 
 struct CorrectorArgs {
+    RawState raw;              // corrector_kernel<true>: the registered fp64 state and the time to predict to
     const float4* gather;      // particle-major predicted records
     int32_t n, n_i;
     const int32_t* i_idx;      // [n_i]
@@ -46,10 +47,11 @@ struct CorrectorArgs {
 };
 
 // One member of a list: its fp32 pair term, added with `sign` to the lane's fp64 sums.
-__device__ __forceinline__ void signed_pair(const PredRecord& pi, const float4* gather, int32_t n, int32_t i,
-                                            int32_t j, double sign, double s[6]) {
+template <bool ACT>
+__device__ __forceinline__ void signed_pair(const PredRecord& pi, const RawState& raw, const float4* gather, int32_t n,
+                                            int32_t i, int32_t j, double sign, double s[6]) {
     if (j == i || j < 0 || j >= n) return;
-    const PredRecord pj = load_record(gather, j);
+    const PredRecord pj = ACT ? predict_record(raw, j) : load_record(gather, j);
     const float dx = (pj.xh - pi.xh) + (pj.xl - pi.xl);
     const float dy = (pj.yh - pi.yh) + (pj.yl - pi.yl);
     const float dz = (pj.zh - pi.zh) + (pj.zl - pi.zl);
@@ -101,12 +103,16 @@ __device__ __forceinline__ bool is_ascending(const int32_t* list, int32_t len, i
     return __all_sync(0xffffffffu, ok);
 }
 
+// ACT: the gathered particles are predicted on the spot from the fp64 state (record.cuh, the paper's PRED_ACT mode,
+// PAPER.md:140), for a small block whose context holds no prediction at t -- e.g. right after a force call that
+// predicted inside the force kernel: the regular step of a small block then runs without any prediction pass.
+template <bool ACT>
 __global__ void __launch_bounds__(kIrrWarps * 32) corrector_kernel(CorrectorArgs a) {
     const int lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * kIrrWarps + (threadIdx.x >> 5);
     if (row >= a.n_i) return;  // warp-uniform
     const int32_t i = a.i_idx[row];
-    const PredRecord pi = load_record(a.gather, i);
+    const PredRecord pi = ACT ? predict_record(a.raw, i) : load_record(a.gather, i);
     const int32_t n_new = a.new_count[row];
     const int32_t len_new = min(n_new, a.new_stride);
     const int32_t len_old = min(a.old_count[row], a.old_stride);
@@ -119,13 +125,13 @@ __global__ void __launch_bounds__(kIrrWarps * 32) corrector_kernel(CorrectorArgs
         const int32_t e = base + lane;
         const int32_t j = (e < len_new) ? lnew[e] : -2;
         const bool common = old_sorted ? in_sorted_list(j, lold, len_old) : in_list(j, lold, len_old, lane);
-        if (!common && j >= 0) signed_pair(pi, a.gather, a.n, i, j, 1.0, s);
+        if (!common && j >= 0) signed_pair<ACT>(pi, a.raw, a.gather, a.n, i, j, 1.0, s);
     }
     for (int32_t base = 0; base < len_old; base += 32) {  // members of L_old that are not in L_new: -
         const int32_t e = base + lane;
         const int32_t j = (e < len_old) ? lold[e] : -2;
         const bool common = new_sorted ? in_sorted_list(j, lnew, len_new) : in_list(j, lnew, len_new, lane);
-        if (!common && j >= 0) signed_pair(pi, a.gather, a.n, i, j, -1.0, s);
+        if (!common && j >= 0) signed_pair<ACT>(pi, a.raw, a.gather, a.n, i, j, -1.0, s);
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {

@@ -719,12 +719,16 @@ int nb_regular_correct(nb_ctx* c, int32_t n_i, const nb_corrector_io* io, double
     if (c->n < 1) return NB_E_STATE;
     NB_CUDA(cudaSetDevice(c->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (!c->predicted || c->t_pred != t) {
+    // as nb_irregular_force: a small block without a prediction at t predicts what it gathers ("irr_pred")
+    const bool stale = !c->predicted || c->t_pred != t;
+    const bool act = c->opt_irr_pred == 2 || (c->opt_irr_pred == 0 && stale && (int64_t)n_i * kIrrActRatio <= c->n);
+    if (stale && !act) {
         int rc = nb_predict_j(c, t, stream);
         if (rc != NB_OK) return rc;
     }
     if (n_i == 0) return NB_OK;
     CorrectorArgs ca{};
+    ca.raw = RawState{c->x0, c->v0, c->a0, c->j0, c->m, c->t0, t};
     ca.gather = reinterpret_cast<const float4*>(c->ws + c->lay.gather_off);
     ca.n = (int32_t)c->n;
     ca.n_i = n_i;
@@ -736,7 +740,8 @@ int nb_regular_correct(nb_ctx* c, int32_t n_i, const nb_corrector_io* io, double
     ca.f1 = io->f1; ca.fd1 = io->fd1; ca.d2 = io->d2; ca.d3 = io->d3; ca.dx = io->dx; ca.dv = io->dv;
     ca.r_s_new = io->r_s_new;
     const unsigned blocks = (unsigned)((n_i + kIrrWarps - 1) / kIrrWarps);
-    corrector_kernel<<<blocks, kIrrWarps * 32, 0, st>>>(ca);
+    if (act) corrector_kernel<true><<<blocks, kIrrWarps * 32, 0, st>>>(ca);
+    else corrector_kernel<false><<<blocks, kIrrWarps * 32, 0, st>>>(ca);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }

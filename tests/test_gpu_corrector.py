@@ -210,3 +210,36 @@ def test_unsorted_lists_take_the_general_path(oracle):
             assert d <= 1e-13 * ref[key].abs().max().item(), (key, d)
     assert (ref["f1"] - new["acc"]).abs().max().item() > 1e-6     # lists differ, the correction is not zero
     ctx.close()
+
+
+def test_small_block_regular_step_runs_without_a_prediction_pass(oracle):
+    """N >= 262144, small block: the force call predicts inside force_kernel, the corrector predicts what it gathers
+    (corrector_kernel<true>): force + gather + corrector = 3 launches per regular step, results identical bit for bit
+    to the chain with the predictor pass."""
+    wl = inputs.make_custom(300001, 96, 30, 128, seed_sub=4, predict=lambda s: oracle.predict_state(s)[0])
+    s = wl.state
+    rs_old = wl.r_s * np.random.default_rng(8).uniform(0.8, 1.2, size=wl.n_i)
+    ctx = binding.Context(s.n, wl.n_i, wl.cap)
+    state_dev = ctx.set_state(s)
+    dev = ctx.workspace.device
+    i_idx = _t(wl.i_idx, dev, np.int32)
+    dt, fr0, frd0, n_p = _step_inputs(wl.n_i, 30, 1.0, 6)
+    res = {}
+    for mode in ("fused", "pass"):
+        ctx.nb_set_option("fuse_pred", 1 if mode == "fused" else 0)
+        ctx.nb_set_option("irr_pred", 0 if mode == "fused" else 1)
+        ctx.nb_set_j(*state_dev)
+        old = ctx.nb_regular_force(i_idx, _t(rs_old, dev), s.t)
+        ctx.nb_set_j(*state_dev)                      # a new step: no prediction in the context
+        new = ctx.nb_regular_force(i_idx, _t(wl.r_s, dev), s.t)
+        launches = ctx.nb_last_launch_info()["launches"]
+        out = ctx.nb_regular_correct(i_idx, _t(dt, dev), _t(fr0, dev), _t(frd0, dev), new["acc"], new["jerk"],
+                                     new["nbr_count"], new["nbr_list"], old["nbr_count"], old["nbr_list"], s.t)
+        torch.cuda.synchronize()
+        res[mode] = (launches, {k: v.clone() for k, v in out.items()}, new["acc"].clone())
+    assert res["fused"][0] == 2 and res["pass"][0] == 3
+    assert torch.equal(res["fused"][2], res["pass"][2])
+    for k in ("f1", "fd1", "d2", "d3", "dx", "dv"):
+        assert torch.equal(res["fused"][1][k], res["pass"][1][k]), k
+    assert (res["fused"][1]["f1"] - res["fused"][2]).abs().max().item() > 0   # the lists differ
+    ctx.close()
