@@ -92,7 +92,7 @@ struct WorkspaceLayout {
 // The j-split workspace holds 7 doubles per (row, chunk): enough slots for 64 chunks per row of the largest
 // block, at least 131072 (small blocks are split hundreds of ways), at most 2M (112 MB).
 int64_t row_chunk_slots(int64_t n_i_max) {
-    return std::min<int64_t>(std::max<int64_t>(64 * n_i_max, 131072), 2097152);
+    return std::min<int64_t>(std::max<int64_t>(256 * n_i_max, 131072), 2097152);
 }
 
 WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {

@@ -23,7 +23,7 @@ def _check_plan(p, n, n_i):
     assert 0 <= tail <= n_blocks and S >= 1
     assert (S == 1) == (tail == 0)
     assert p["ctas"] == (n_blocks - tail) + tail * S
-    assert tail * rows * S <= min(max(64 * n_i, 131072), 2097152)  # (row, chunk) slots of the j-split workspace
+    assert tail * rows * S <= min(max(256 * n_i, 131072), 2097152)  # (row, chunk) slots of the j-split workspace
     if S > 1:  # the chunks cover the tiles exactly, none is empty
         tpc = p["tiles_per_chunk"]
         assert (S - 1) * tpc < n_tiles <= S * tpc
