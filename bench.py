@@ -169,8 +169,8 @@ def workload_config(wl, config):
                         f"k~{wl.k}, nbr cap {wl.cap}", "n": wl.state.n, "n_i": wl.n_i, "nbr_cap": wl.cap,
             "pairs_per_step": wl.pairs, "flops_per_pair_convention": FLOPS_PER_PAIR,
             "r_s_calibrated_on": wl.rs_positions,
-            "l2": "no explicit flush: each step streams 112 B/j of fp64 state plus outputs "
-                  "(lists N_i x cap x 4 B), larger than the 126 MB L2 for the default workload"}
+            "l2": "a 256 MiB device fill (> the 126 MB L2) flushes L2 before every timed step, outside the per-step "
+                  "events (--sweep rows: back-to-back calls, no flush)"}
 
 
 def run_sweep(args):

@@ -15,7 +15,10 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-pointer calls only
  *     ENQUEUE work on `stream` and return; they never synchronise the host.
  *   - [n][3] arrays are row-major (x, y, z contiguous per particle).  Indices are 0-based int32.
- *   - Every function returns NB_OK (0) or a negative NB_E_* code; on error nothing has been enqueued.
+ *   - Every function returns NB_OK (0) or a negative NB_E_* code.  Argument and state errors (NB_E_INVAL, NB_E_STATE,
+ *     NB_E_NOMEM) are found before anything is enqueued.  A call enqueues several kernels; if a later launch fails
+ *     (NB_E_CUDA) the work already enqueued is NOT rolled back and the outputs are undefined.  nb_regular_force_host
+ *     synchronises its internal streams before it returns, on the error paths too.
  *     nb_strerror() gives the text; for NB_E_CUDA it includes the CUDA error string of the last failure.
  *   - A context is not thread-safe and owns ONE workspace: issue its calls from one thread at a time and keep them
  *     on one stream (or order streams yourself); use one context per concurrent stream.
@@ -77,8 +80,11 @@ int nb_set_j(nb_ctx* ctx, int64_t n, const double* x0, const double* v0, const d
  * (hi = fl32(x_p), lo = fl32(x_p - hi)), velocity and mass as fl32.  Enqueues one kernel on `stream`. */
 int nb_predict_j(nb_ctx* ctx, double t, void* stream);
 
-/* Test hook: write the fp64 predicted state of the last nb_predict_j / nb_regular_force time to
- * xp, vp: dev double[n][3].  Same kernel and arithmetic as nb_predict_j. */
+/* Test hook: write the fp64 predicted state at the time of the last prediction PASS (nb_predict_j, or the pass a
+ * force / irregular / corrector call ran first) to xp, vp: dev double[n][3].  Same kernel and arithmetic as
+ * nb_predict_j.  A call that predicted inside its own kernel (small blocks: options "fuse_pred", "irr_pred") leaves
+ * no prediction in the context: this function then returns NB_E_STATE, or the state of an older pass if the context
+ * still holds one -- call nb_predict_j(t) first to be sure of t. */
 int nb_get_predicted(nb_ctx* ctx, double* xp, double* vp, void* stream);
 
 /* Step (vi), eq. (9), (10), (11), with the plain neighbour criterion eq. (2), PAPER.md:65-67:
@@ -203,6 +209,20 @@ int nb_regular_force_host(nb_ctx* ctx, int64_t n, const double* x0, const double
                           const double* j0, const double* m, const double* t0, int32_t n_i, const int32_t* i_idx,
                           const double* r_s, double t, double* acc, double* jerk, int32_t* nbr_count,
                           int32_t* nbr_list, int32_t* n_overflow);
+
+/* The fp64 fix-up pass (footnote 2: "options using the 'two-float' method for the coordinates and the
+ * accumulator").  The pair arithmetic of nb_regular_force[_ex] is fp32, so a row's absolute error is
+ * ~ eps sqrt(sum_j |term_j|^2) whatever its sum comes to; rows whose terms cancel would miss the per-particle bound
+ * (1e-6 |acc|, 1e-5 |jerk|).  The force kernel estimates that scale per row for free (squared norms of its per-tile
+ * partial sums: q_a, q_j); a row with C_a sqrt(q_a) > |acc| or C_j sqrt(q_j) > |jerk| is evaluated again in fp64 by one
+ * more kernel of the same call, over exactly the complement of the list the fp32 kernel emitted (its neighbour tests
+ * are repeated bit for bit).  Options: "fixup" 0 | 1 (default 1); "fixup_ca_milli", "fixup_cj_milli" = 1000 C_a, 1000 C_j.
+ *
+ * nb_get_error_scale: test hook.  escale: dev float[n_i][2] = (q_a, q_j) of rows 0 .. n_i-1 of the last force call.
+ * nb_fixup_stats: stats (HOST int64[2]) = rows the last force call recomputed in fp64, rows recomputed since nb_create.
+ *                 Synchronises `stream`. */
+int nb_get_error_scale(nb_ctx* ctx, int32_t n_i, float* escale, void* stream);
+int nb_fixup_stats(nb_ctx* ctx, int64_t stats[2], void* stream);
 
 /* Tuning knobs (tests and benchmarks).  key:
  *   "j_split"   force the number of j-chunks per row for ALL row blocks (0 = automatic; 1 = never split)

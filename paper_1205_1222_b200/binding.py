@@ -54,6 +54,8 @@ def load(build_if_missing: bool = True):
     lib.nb_regular_correct.argtypes = [vp, i32, ctypes.POINTER(CorrectorIO), dbl, vp]
     lib.nb_regular_force_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp]
     lib.nb_set_option.argtypes = [vp, ctypes.c_char_p, i64]
+    lib.nb_get_error_scale.argtypes = [vp, i32, vp, vp]
+    lib.nb_fixup_stats.argtypes = [vp, ctypes.POINTER(i64), vp]
     lib.nb_last_launch_info.argtypes = [vp, ctypes.POINTER(i64)]
     lib.nb_plan.argtypes = [i64, i32, i32, ctypes.POINTER(i32), i64, i64, ctypes.POINTER(i64)]
     _lib = lib
@@ -249,6 +251,18 @@ class Context:
 
     def nb_set_option(self, key: str, value: int):
         _check(self.lib.nb_set_option(self._h, key.encode(), int(value)))
+
+    def nb_get_error_scale(self, n_i: int, stream=None):
+        """Test hook: (q_a, q_j) per row of the last force call, float32 [n_i][2]."""
+        out = torch.empty((int(n_i), 2), dtype=torch.float32, device=self.workspace.device)
+        _check(self.lib.nb_get_error_scale(self._h, int(n_i), ctypes.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+        return out
+
+    def nb_fixup_stats(self, stream=None) -> dict:
+        """Rows the last force call recomputed in fp64, and since nb_create (synchronises the stream)."""
+        arr = (ctypes.c_int64 * 2)()
+        _check(self.lib.nb_fixup_stats(self._h, arr, _stream_ptr(stream)))
+        return dict(last=int(arr[0]), total=int(arr[1]))
 
     def nb_last_launch_info(self) -> dict:
         arr = (ctypes.c_int64 * 8)()

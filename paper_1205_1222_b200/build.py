@@ -2,15 +2,21 @@
 from __future__ import annotations
 
 import os
+import glob
 import shutil
 import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "nbreg_api.cu")
-DEPS = [os.path.join(HERE, "csrc", f) for f in
-        ("nbreg_api.cu", "nbreg_common.cuh", "predict.cuh", "force.cuh", "gather.cuh", "irregular.cuh", "order.cuh")] + \
-       [os.path.join(os.path.dirname(HERE), "include", "nbreg.h")]
+INCLUDE = os.path.join(os.path.dirname(HERE), "include", "nbreg.h")
+
+
+def deps() -> list:
+    """Every source the one translation unit includes: all of csrc/ (globbed, so a new header cannot be forgotten)."""
+    return sorted(glob.glob(os.path.join(HERE, "csrc", "*.cu")) + glob.glob(os.path.join(HERE, "csrc", "*.cuh"))) + [INCLUDE]
+
+
 LIB = os.environ.get("NBREG_LIB") or os.path.join(HERE, "libnbreg.so")  # NBREG_LIB: use a library built elsewhere
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
@@ -28,7 +34,7 @@ def stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(d) > t for d in DEPS)
+    return any(os.path.getmtime(d) > t for d in deps())
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

@@ -1,0 +1,208 @@
+// fixup.cuh -- the fp64 fix-up pass: rows of eq. (9), (10) whose sum is dominated by cancellation
+// are evaluated again with fp64 pair arithmetic, so that the per-particle bound (1e-6 |acc|, 1e-5 |jerk|) holds for
+// every row and not only for the typical one.  Which rows: fixflag.cuh (queued by force_kernel / the gather kernels;
+// a few per 10^4 at the paper's workloads).  The paper's own answer to the same problem is footnote 2, PAPER.md:154:
+// "there remain options using the 'two-float' method for the coordinates and the accumulator".
+//
+// The neighbour decisions are NOT taken again: a pair is left out of the fp64 sums iff the fp32 test of force_kernel's
+// near path (geom_hi + geom_lo [+ rmin2_velocity], the same device functions on the same fp32 records) calls it a
+// neighbour, so the result stays the sum over exactly the complement of the emitted list.  (A pair force_kernel took
+// on its far path is never a neighbour by that test either: the far threshold carries a 2^-10 margin, force.cuh.)
+//
+// Mapping: the queued rows are taken eight at a time (one row per warp); a work item is (group of 8 rows, j-chunk).
+// The 256 threads of a CTA predict a tile of 256 j straight from the registered fp64 state into shared memory (the
+// Horner form of predict.cuh; fp64 x_p, v_p, m and the fp32 record the neighbour test needs), then every warp runs its
+// row over the tile, lanes striding over j.  Lane sums are fp64, reduced by a fixed xor-shuffle tree; the chunks of a
+// row are added in a fixed order by the CTA that finishes last (atomic ticket): deterministic for a given device.
+// The pass always runs (one launch); with nothing queued every CTA returns at once.
+#pragma once
+#include "fixflag.cuh"
+#include "force.cuh"
+#include "record.cuh"
+
+namespace nbreg {
+
+constexpr int kFixWarps = 8;                 // rows per group = warps per CTA
+constexpr int kFixThreads = kFixWarps * 32;  // = j per tile
+constexpr int kFixMaxGrid = 1024;
+
+struct FixupArgs {
+    RawState raw;
+    int32_t n;
+    const int32_t* i_idx;
+    const double* r_s;
+    const double* dtr;       // VEL: regular time-step per row (eq. (3)), else null
+    double* acc;
+    double* jerk;
+    int32_t* count;          // [1] queued rows (zero between calls; re-zeroed here)
+    const int32_t* rows;     // [count] the caller's rows
+    double* part;            // [(group, chunk)][kFixWarps][6] partial sums of the j-chunks
+    int32_t* tickets;        // [groups] chunks of the group that are done (zero between calls)
+    int32_t* done;           // [1] CTAs of this launch that are done (zero between calls)
+    int32_t* stat_last;      // [1] rows the last call recomputed
+    unsigned long long* stat_total;  // [1] rows recomputed since nb_create
+};
+
+template <bool VEL>
+__global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
+    __shared__ double sx[3][kFixThreads], sv[3][kFixThreads], sm[kFixThreads];
+    __shared__ float sh[3][kFixThreads], sl[3][kFixThreads], sw[3][kFixThreads];
+    __shared__ int s_last;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int32_t n_fix = *reinterpret_cast<volatile int32_t*>(a.count);
+    if (n_fix == 0) {  // the usual case
+        if (blockIdx.x == 0 && tid == 0) *a.stat_last = 0;
+        return;
+    }
+    const int32_t groups = (n_fix + kFixWarps - 1) / kFixWarps;
+    const int32_t n_tiles = (a.n + kFixThreads - 1) / kFixThreads;
+    int32_t C = min(((int32_t)gridDim.x + groups - 1) / groups, n_tiles);  // j-chunks per group: enough items for the grid
+    const int32_t tpc = (n_tiles + C - 1) / C;
+    C = (n_tiles + tpc - 1) / tpc;
+    const int64_t items = (int64_t)groups * C;
+
+    for (int64_t item = blockIdx.x; item < items; item += gridDim.x) {
+        const int32_t g = (int32_t)(item / C), c = (int32_t)(item % C);
+        const int32_t f = g * kFixWarps + warp;
+        const bool live = f < n_fix;  // warp-uniform
+        // ---- this warp's row: predicted in fp64, and its fp32 record exactly as force_kernel's i-setup forms it
+        int32_t orow = 0, i = 0;
+        double xi[3] = {0.0, 0.0, 0.0}, vi[3] = {0.0, 0.0, 0.0};
+        IState I{};
+        if (live) {
+            orow = a.rows[f];
+            i = a.i_idx[orow];
+            const double dt = a.raw.t - __ldg(a.raw.t0 + i);
+            float h[3], l[3], w[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const double x = __ldg(a.raw.x0 + 3 * (size_t)i + k), v = __ldg(a.raw.v0 + 3 * (size_t)i + k);
+                const double ac = __ldg(a.raw.a0 + 3 * (size_t)i + k), jk = __ldg(a.raw.j0 + 3 * (size_t)i + k);
+                xi[k] = x + dt * (v + dt * (0.5 * ac + dt * ((1.0 / 6.0) * jk)));
+                vi[k] = v + dt * (ac + dt * (0.5 * jk));
+                h[k] = __double2float_rn(xi[k]);
+                l[k] = __double2float_rn(xi[k] - (double)h[k]);
+                w[k] = __double2float_rn(vi[k]);
+            }
+            I.nxh = -h[0]; I.nyh = -h[1]; I.nzh = -h[2];
+            I.nxl = -l[0]; I.nyl = -l[1]; I.nzl = -l[2];
+            I.nvx = -w[0]; I.nvy = -w[1]; I.nvz = -w[2];
+            const double rs = a.r_s[orow];
+            I.h2 = fmaxf(__double2float_rn(rs * rs), 1.17549435e-38f);
+            I.dtr = VEL ? __double2float_rn(a.dtr[orow]) : 0.f;
+        }
+        double s[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        const int32_t t_end = min((c + 1) * tpc, n_tiles);
+        for (int32_t t = c * tpc; t < t_end; ++t) {
+            __syncthreads();  // the previous tile has been read by every warp
+            {
+                const int32_t j = t * kFixThreads + tid;
+                if (j < a.n) {
+                    const double dt = a.raw.t - __ldg(a.raw.t0 + j);
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) {
+                        const double x = __ldg(a.raw.x0 + 3 * (size_t)j + k), v = __ldg(a.raw.v0 + 3 * (size_t)j + k);
+                        const double ac = __ldg(a.raw.a0 + 3 * (size_t)j + k), jk = __ldg(a.raw.j0 + 3 * (size_t)j + k);
+                        const double xp = x + dt * (v + dt * (0.5 * ac + dt * ((1.0 / 6.0) * jk)));
+                        const double vp = v + dt * (ac + dt * (0.5 * jk));
+                        const float xh = __double2float_rn(xp);
+                        sx[k][tid] = xp;
+                        sv[k][tid] = vp;
+                        sh[k][tid] = xh;
+                        sl[k][tid] = __double2float_rn(xp - (double)xh);
+                        sw[k][tid] = __double2float_rn(vp);
+                    }
+                    sm[tid] = __ldg(a.raw.m + j);
+                }
+            }
+            __syncthreads();
+            if (!live) continue;
+            const int32_t jn = min(kFixThreads, a.n - t * kFixThreads);
+            for (int32_t jj = lane; jj < jn; jj += 32) {
+                const int32_t j = t * kFixThreads + jj;
+                if (j == i) continue;
+                // the neighbour test of force_kernel's near path, on the same fp32 words (both halves hold j)
+                const float4 q0 = make_float4(sh[0][jj], sh[0][jj], sh[1][jj], sh[1][jj]);
+                const float4 q1 = make_float4(sh[2][jj], sh[2][jj], 0.f, 0.f);
+                const float4 q2 = make_float4(sw[0][jj], sw[0][jj], sw[1][jj], sw[1][jj]);
+                const float2 vz = make_float2(sw[2][jj], sw[2][jj]);
+                const float2 xl = make_float2(sl[0][jj], sl[0][jj]);
+                const float4 q4 = make_float4(sl[1][jj], sl[1][jj], sl[2][jj], sl[2][jj]);
+                PairGeom gm;
+                geom_hi(q0, q1, I, gm);
+                geom_lo(xl, q4, I, gm);
+                const float2 rm = VEL ? rmin2_velocity(q2, vz, I, gm) : gm.r2;
+                if (rm.x < I.h2) continue;  // neighbour: listed by force_kernel, not summed
+                // eq. (9), (10) in fp64
+                const double Rx = sx[0][jj] - xi[0], Ry = sx[1][jj] - xi[1], Rz = sx[2][jj] - xi[2];
+                const double Vx = sv[0][jj] - vi[0], Vy = sv[1][jj] - vi[1], Vz = sv[2][jj] - vi[2];
+                const double r2 = Rx * Rx + Ry * Ry + Rz * Rz;
+                if (r2 == 0.0) continue;  // coincident (reading R4)
+                const double ri = rsqrt(r2), ri2 = ri * ri;
+                const double mri3 = sm[jj] * ri * ri2;
+                const double al = -3.0 * (Rx * Vx + Ry * Vy + Rz * Vz) * ri2;
+                s[0] += mri3 * Rx;
+                s[1] += mri3 * Ry;
+                s[2] += mri3 * Rz;
+                s[3] += mri3 * (Vx + al * Rx);
+                s[4] += mri3 * (Vy + al * Ry);
+                s[5] += mri3 * (Vz + al * Rz);
+            }
+        }
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+#pragma unroll
+            for (int k = 0; k < 6; ++k) s[k] += __shfl_xor_sync(0xffffffffu, s[k], off);
+        }
+        if (C == 1) {
+            if (live && lane < 3) {
+                a.acc[(size_t)orow * 3 + lane] = (lane == 0) ? s[0] : (lane == 1) ? s[1] : s[2];
+                a.jerk[(size_t)orow * 3 + lane] = (lane == 0) ? s[3] : (lane == 1) ? s[4] : s[5];
+            }
+            continue;
+        }
+        if (live && lane == 0) {
+            double* ps = a.part + ((size_t)item * kFixWarps + warp) * 6;
+#pragma unroll
+            for (int k = 0; k < 6; ++k) ps[k] = s[k];
+        }
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) s_last = (atomicAdd(a.tickets + g, 1) == C - 1);
+        __syncthreads();
+        if (s_last) {  // every chunk of this group is in: lanes stride over the chunks, then the fixed shuffle tree
+            __threadfence();
+            if (live) {
+                double v[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+                for (int32_t cc = lane; cc < C; cc += 32) {
+                    const double* ps = a.part + (((size_t)g * C + cc) * kFixWarps + warp) * 6;
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) v[k] += __ldcg(ps + k);
+                }
+#pragma unroll
+                for (int off = 16; off > 0; off >>= 1) {
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) v[k] += __shfl_xor_sync(0xffffffffu, v[k], off);
+                }
+                if (lane < 3) {
+                    a.acc[(size_t)orow * 3 + lane] = (lane == 0) ? v[0] : (lane == 1) ? v[1] : v[2];
+                    a.jerk[(size_t)orow * 3 + lane] = (lane == 0) ? v[3] : (lane == 1) ? v[4] : v[5];
+                }
+            }
+            if (tid == 0) a.tickets[g] = 0;
+        }
+    }
+    // ---- the last CTA to finish leaves the queue empty for the next call
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        if (atomicAdd(a.done, 1) == (int32_t)gridDim.x - 1) {
+            *a.count = 0;
+            *a.done = 0;
+            *a.stat_last = n_fix;
+            *a.stat_total += (unsigned long long)n_fix;
+        }
+    }
+}
+
+}  // namespace nbreg

@@ -25,6 +25,7 @@
 #pragma once
 #include "nbreg_common.cuh"
 #include "record.cuh"
+#include "fixflag.cuh"
 
 namespace nbreg {
 
@@ -66,9 +67,11 @@ struct ForceArgs {
     // zero-between-calls scratch in the workspace (reduce_gather_kernel leaves it zeroed again):
     int32_t* slot_count;    // [tail rows] list-slot counters of the j-split rows
     int32_t* overflow_ws;   // [1] rows with count > cap found so far in this call
-    // partial sums of the tail blocks, indexed by tail row = row - main_blocks * rows_per_cta: [tail row][S][6].
-    // Their list entries go straight to nbr_list through the atomic slot counters slot_count.
+    // partial sums of the tail blocks, indexed by tail row = row - main_blocks * rows_per_cta: [tail row][S][kSums + 1]
+    // (the last slot holds the two error-scale sums as a float2).  Their list entries go straight to nbr_list through
+    // the atomic slot counters slot_count.
     double* part_sum;
+    FixupFlag fix;          // rows whose result is dominated by cancellation are queued for fixup_kernel (fixup.cuh)
 };
 
 // ---------------------------------------------------------------- PTX helpers
@@ -270,7 +273,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
     constexpr int kRows = kThreads * IPT;
     constexpr int kTileQuads = JT / 2 * kQuadsPerPair;
     constexpr uint32_t kTileBytes = JT * kBytesPerJ;
-    constexpr int kStages = 2;
+    constexpr int kStages = PRED ? 1 : 2;  // the fused-prediction variant fills its one stage itself
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float4* tiles = reinterpret_cast<float4*>(smem_raw);
@@ -278,8 +281,12 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
     // The fp64 running sums (S6) live in shared memory, [component][i-of-thread][thread]: they are touched once per
     // j-tile, and without their 12 registers per i the kernel fits 64 registers = 32 resident warps per SM
     // (measured: 1108 -> 1140 Gpairs/s at config 5).
-    double* ssum = reinterpret_cast<double*>(smem_raw + kStages * kTileBytes + kStages * sizeof(uint64_t));
+    double* ssum = reinterpret_cast<double*>(smem_raw + kStages * kTileBytes + 2 * sizeof(uint64_t));
 #define NB_SUM(u, c) ssum[((c) * IPT + (u)) * kThreads + tid]
+    // Error scale of the row (fixup.cuh): the squared norms of the per-tile fp32 partial sums, added up over the
+    // tiles -- sum_T |acc_T|^2 and sum_T |jerk_T|^2.  Touched once per tile, like the running sums.
+    float2* sq = reinterpret_cast<float2*>(ssum + kSums * kRows);
+#define NB_Q(u) sq[(u) * kThreads + tid]
 
     const int tid = threadIdx.x;
     const bool split = (int)blockIdx.x >= a.main_blocks;
@@ -352,6 +359,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         accum_zero(s[u]);
 #pragma unroll
         for (int c = 0; c < kSums; ++c) NB_SUM(u, c) = 0.0;
+        NB_Q(u) = make_float2(0.f, 0.f);
     }
 
     // ---- S3/S4: stream the j-tiles
@@ -425,14 +433,33 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         // ---- S6: flush the tile's fp32 partial sums into the fp64 running sums
 #pragma unroll
         for (int u = 0; u < IPT; ++u) {
-            NB_SUM(u, 0) += (double)s[u].ax.x + (double)s[u].ax.y;
-            NB_SUM(u, 1) += (double)s[u].ay.x + (double)s[u].ay.y;
-            NB_SUM(u, 2) += (double)s[u].az.x + (double)s[u].az.y;
-            NB_SUM(u, 3) += (double)s[u].jx.x + (double)s[u].jx.y;
-            NB_SUM(u, 4) += (double)s[u].jy.x + (double)s[u].jy.y;
-            NB_SUM(u, 5) += (double)s[u].jz.x + (double)s[u].jz.y;
-            if (POT) NB_SUM(u, kSums - 1) += (double)s[u].pot.x + (double)s[u].pot.y;
-            accum_zero(s[u]);
+            // Error scale: a tile's partial sums are sums of ~JT terms of mixed direction, so their squared norms add up
+            // (over the tiles) to an estimate of sum_j |term_j|^2, the variance scale of the row's fp32 rounding error
+            // (fixflag.cuh).  Component by component, so that no more registers are live than without it.
+#define NB_FLUSH(c, f, qq)                                    \
+    {                                                         \
+        const float t = (f).x + (f).y;                        \
+        NB_SUM(u, c) += (double)(f).x + (double)(f).y;        \
+        (f) = make_float2(0.f, 0.f);                          \
+        qq = fmaf(t, t, qq);                                  \
+    }
+            // (shared-memory reductions instead of a read-modify-write through registers: the kernel keeps its 64
+            // registers = 32 resident warps per SM; with q in registers across the flush ptxas needs 68)
+            float qq = 0.f;
+            NB_FLUSH(0, s[u].ax, qq)
+            NB_FLUSH(1, s[u].ay, qq)
+            NB_FLUSH(2, s[u].az, qq)
+            atomicAdd(&NB_Q(u).x, qq);
+            qq = 0.f;
+            NB_FLUSH(3, s[u].jx, qq)
+            NB_FLUSH(4, s[u].jy, qq)
+            NB_FLUSH(5, s[u].jz, qq)
+            atomicAdd(&NB_Q(u).y, qq);
+#undef NB_FLUSH
+            if (POT) {
+                NB_SUM(u, kSums - 1) += (double)s[u].pot.x + (double)s[u].pot.y;
+                s[u].pot = make_float2(0.f, 0.f);
+            }
         }
         if (WARPS > 1) __syncthreads(); else __syncwarp();  // every warp is done with stage st before it is refilled
     }
@@ -452,16 +479,21 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
             if (POT) a.pot[orow] = NB_SUM(u, kSums - 1);
             a.nbr_count[orow] = I[u].cnt;
             if (I[u].cnt > a.cap) atomicAdd(a.overflow_ws, 1);
+            const float2 q = NB_Q(u);
+            fixup_flag(a.fix, (int32_t)orow, q.x, q.y, NB_SUM(u, 0), NB_SUM(u, 1), NB_SUM(u, 2), NB_SUM(u, 3),
+                       NB_SUM(u, 4), NB_SUM(u, 5));
         } else {
             flush_pending(I[u], a.cap);
             const size_t pi = (size_t)(row - tail_row0) * a.n_chunks + chunk;
-            double* ps = a.part_sum + pi * kSums;
+            double* ps = a.part_sum + pi * (kSums + 1);
 #pragma unroll
             for (int c = 0; c < kSums; ++c) ps[c] = NB_SUM(u, c);
+            *reinterpret_cast<float2*>(ps + kSums) = NB_Q(u);
         }
     }
 }
 
 #undef NB_SUM
+#undef NB_Q
 
 }  // namespace nbreg

@@ -13,6 +13,7 @@
 //   second pass writes every entry to offset[chunk] + its rank among earlier entries of the same chunk.  O(count + S).
 #pragma once
 #include "nbreg_common.cuh"
+#include "fixflag.cuh"
 
 namespace nbreg {
 
@@ -23,7 +24,8 @@ struct GatherArgs {
     int32_t n_chunks;
     int32_t chunk_j;           // j-particles per chunk (tiles_per_chunk * j-tile)
     int32_t cap;
-    const double* part_sum;    // [split rows][S][6], or [..][7] with the potential
+    const double* part_sum;    // [split rows][S][7], or [..][8] with the potential: acc, jerk (, pot), error scales (float2)
+    FixupFlag fix;             // rows dominated by cancellation are queued for fixup_kernel (fixflag.cuh)
     double* acc;
     double* jerk;
     double* pot;               // null: no potential (6 partial sums per chunk), else 7
@@ -51,23 +53,30 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
 
     // ---- partial sums (fixed order: chunk = lane, lane + 32, ...; then xor tree 16, 8, 4, 2, 1)
     double s[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    float qa = 0.f, qj = 0.f;  // error scales of the chunks (fixflag.cuh)
     const int n_sums = a.pot ? 7 : 6;
     for (int c = lane; c < S; c += 32) {
-        const double* ps = a.part_sum + (rbase + c) * n_sums;
+        const double* ps = a.part_sum + (rbase + c) * (n_sums + 1);
 #pragma unroll
         for (int k = 0; k < 7; ++k)
             if (k < n_sums) s[k] += ps[k];
+        const float2 q = *reinterpret_cast<const float2*>(ps + n_sums);
+        qa += q.x;
+        qj += q.y;
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
 #pragma unroll
         for (int k = 0; k < 7; ++k) s[k] += __shfl_xor_sync(0xffffffffu, s[k], off);
+        qa += __shfl_xor_sync(0xffffffffu, qa, off);
+        qj += __shfl_xor_sync(0xffffffffu, qj, off);
     }
     if (lane == 0 && a.pot) a.pot[orow] = s[6];
     if (lane < 3) {
         a.acc[orow * 3 + lane] = (lane == 0) ? s[0] : (lane == 1) ? s[1] : s[2];
         a.jerk[orow * 3 + lane] = (lane == 0) ? s[3] : (lane == 1) ? s[4] : s[5];
     }
+    if (lane == 0) fixup_flag(a.fix, (int32_t)orow, qa, qj, s[0], s[1], s[2], s[3], s[4], s[5]);
 
     // ---- list: stable counting sort of the stored entries by chunk number
     const int32_t cnt = a.slot_count[prow];  // true count, may exceed cap
@@ -149,6 +158,8 @@ constexpr int64_t kWideFewRows = 296;
 __global__ void __launch_bounds__(kWideThreadsFew) reduce_gather_wide_kernel(GatherArgs a) {
     extern __shared__ int32_t stage[];  // cap entries
     __shared__ double warp_sum[kWideThreadsFew / 32][7];
+    __shared__ float2 warp_q[kWideThreadsFew / 32];
+    __shared__ double row_sum[6];
     const int n_threads = blockDim.x;  // kWideThreads or kWideThreadsFew
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t prow = blockIdx.x;
@@ -158,21 +169,28 @@ __global__ void __launch_bounds__(kWideThreadsFew) reduce_gather_wide_kernel(Gat
     const size_t rbase = (size_t)prow * S;
 
     double s[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    float qa = 0.f, qj = 0.f;  // error scales of the chunks (fixflag.cuh)
     const int n_sums = a.pot ? 7 : 6;
     for (int c = tid; c < S; c += n_threads) {
-        const double* ps = a.part_sum + (rbase + c) * n_sums;
+        const double* ps = a.part_sum + (rbase + c) * (n_sums + 1);
 #pragma unroll
         for (int k = 0; k < 7; ++k)
             if (k < n_sums) s[k] += ps[k];
+        const float2 q = *reinterpret_cast<const float2*>(ps + n_sums);
+        qa += q.x;
+        qj += q.y;
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
 #pragma unroll
         for (int k = 0; k < 7; ++k) s[k] += __shfl_xor_sync(0xffffffffu, s[k], off);
+        qa += __shfl_xor_sync(0xffffffffu, qa, off);
+        qj += __shfl_xor_sync(0xffffffffu, qj, off);
     }
     if (lane == 0) {
 #pragma unroll
         for (int k = 0; k < 7; ++k) warp_sum[warp][k] = s[k];
+        warp_q[warp] = make_float2(qa, qj);
     }
     const int32_t cnt = a.slot_count[prow];  // true count, may exceed cap
     const int32_t stored = min(cnt, a.cap);
@@ -185,6 +203,7 @@ __global__ void __launch_bounds__(kWideThreadsFew) reduce_gather_wide_kernel(Gat
         if (tid < 3) a.acc[row * 3 + tid] = v;
         else if (tid < 6) a.jerk[row * 3 + tid - 3] = v;
         else a.pot[row] = v;
+        if (tid < 6) row_sum[tid] = v;
     }
     for (int32_t e = tid; e < stored; e += n_threads) {
         const int32_t v = stage[e];
@@ -197,6 +216,12 @@ __global__ void __launch_bounds__(kWideThreadsFew) reduce_gather_wide_kernel(Gat
         a.nbr_count[row] = cnt;
         a.slot_count[prow] = 0;
         if (cnt > a.cap) atomicAdd(a.overflow_ws, 1);
+        float qa = 0.f, qj = 0.f;
+        for (int w = 0; w < n_threads / 32; ++w) {  // fixed order
+            qa += warp_q[w].x;
+            qj += warp_q[w].y;
+        }
+        fixup_flag(a.fix, (int32_t)row, qa, qj, row_sum[0], row_sum[1], row_sum[2], row_sum[3], row_sum[4], row_sum[5]);
         __threadfence();
         if (atomicAdd(a.ticket, 1) == (int32_t)gridDim.x - 1) {
             *a.n_overflow = atomicExch(a.overflow_ws, 0);

@@ -12,6 +12,7 @@
 #include <new>
 
 #include "force.cuh"
+#include "fixup.cuh"
 #include "gather.cuh"
 #include "irregular.cuh"
 #include "corrector.cuh"
@@ -83,13 +84,18 @@ struct WorkspaceLayout {
     size_t vmax_off, vmax_bytes;   // float speed bound per 256 consecutive j (predictor -> velocity criterion)
     size_t sort_off, sort_bytes;   // row ordering: keys and rows, two buffers each, + the library sort's scratch
     size_t sort_temp_bytes;
+    size_t fixrow_off, fixrow_bytes;  // int32 caller's rows queued for the fp64 fix-up pass (fixup.cuh)
+    size_t escale_off, escale_bytes;  // float2 error scales per caller's row (fixflag.cuh)
     size_t slot_off, slot_bytes;   // int32 list-slot counters of the j-split rows (zero between calls)
-    size_t ctl_off, ctl_bytes;     // int32 {overflow count, gather ticket, order ticket, -, 6 box words} (zero between calls)
+    size_t ftick_off, ftick_bytes; // int32 chunk tickets of the fix-up groups (zero between calls)
+    // int32 {overflow count, gather ticket, order ticket, -, 6 box words, -, -, -, -, -, -, fix-up queue length, fix-up
+    // CTA ticket} (zero between calls), then {rows of the last fix-up, -, rows since nb_create (64 bit)}
+    size_t ctl_off, ctl_bytes;
     int64_t row_chunk_limit;  // (row, j-chunk) slots of partial sums
     size_t total;
 };
 
-// The j-split workspace holds 7 doubles per (row, chunk): enough slots for 64 chunks per row of the largest
+// The j-split workspace holds 7 doubles per (row, chunk): enough slots for 256 chunks per row of the largest
 // block, at least 131072 (small blocks are split hundreds of ways), at most 2M (112 MB).
 int64_t row_chunk_slots(int64_t n_i_max) {
     return std::min<int64_t>(std::max<int64_t>(256 * n_i_max, 131072), 2097152);
@@ -107,7 +113,11 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
         off += (size_t)round_up((int64_t)bytes, 256);
     };
     place((size_t)n_pad * kBytesPerJ, w.packed_off, w.packed_bytes);
-    place((size_t)w.row_chunk_limit * 7 * sizeof(double), w.psum_off, w.psum_bytes);  // acc, jerk, pot
+    // acc, jerk, pot, error scales per (row, chunk); the fix-up pass, which runs after the gather, keeps the partial sums
+    // of its (group, chunk) items in the same region: fewer than grid + groups items of kFixWarps x 6 doubles
+    place(std::max((size_t)w.row_chunk_limit * 8 * sizeof(double),
+                   ((size_t)kFixMaxGrid * kFixWarps + (size_t)n_i_max + kFixWarps) * 6 * sizeof(double)),
+          w.psum_off, w.psum_bytes);
     place((size_t)n_pad * kGatherQuads * sizeof(float4), w.gather_off, w.gather_bytes);
     place((size_t)(n_pad / kJPad) * sizeof(float), w.vmax_off, w.vmax_bytes);
     {
@@ -119,13 +129,21 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
         w.sort_temp_bytes = (size_t)round_up((int64_t)temp, 256) + 256;
         place(4 * (size_t)round_up(ni * 4, 256) + w.sort_temp_bytes, w.sort_off, w.sort_bytes);
     }
+    place((size_t)(n_i_max + 1) * sizeof(int32_t), w.fixrow_off, w.fixrow_bytes);
+    place((size_t)(n_i_max + 1) * sizeof(float2), w.escale_off, w.escale_bytes);
     place((size_t)(n_i_max + 512) * sizeof(int32_t), w.slot_off, w.slot_bytes);
-    place(64, w.ctl_off, w.ctl_bytes);
+    place((size_t)(n_i_max / kFixWarps + 2) * sizeof(int32_t), w.ftick_off, w.ftick_bytes);
+    place(128, w.ctl_off, w.ctl_bytes);
     w.total = off;
     return w;
 }
 
 }  // namespace
+
+// Default thresholds of the fp64 fix-up (calibrated against the fp64 oracle on every row of
+// configs 3 and 5): a row's fp32 error is ~ eps sqrt(q) with eps up to ~1e-6 in the far tail, so C = S eps / tolerance.
+constexpr int64_t kFixCaMilli = 2000;  // C_a = 2.0
+constexpr int64_t kFixCjMilli = 200;   // C_j = 0.2
 
 // nb_regular_force_host splits large active blocks into up to kHostChunks row chunks so that the device-to-host copy
 // of one chunk's outputs (the list array dominates) runs while the next chunk is computed
@@ -136,6 +154,7 @@ struct nb_ctx {
     int device = 0;
     int num_sms = 0;
     int ctas_per_sm[4][kNumShapes] = {};  // resident CTAs per SM of each force-kernel variant and shape
+    int ctas_per_sm_pred[kNumShapes] = {}; // ... of the fused-prediction variant (shapes 1-3; others 0)
     int64_t n_max = 0, n_i_max = 0;
     int32_t cap = 0;
     unsigned char* ws = nullptr;
@@ -146,8 +165,15 @@ struct nb_ctx {
     const double *x0 = nullptr, *v0 = nullptr, *a0 = nullptr, *j0 = nullptr, *m = nullptr, *t0 = nullptr;
     bool predicted = false;
     double t_pred = 0.0;
+    // the particle-major copy of the predicted records (gathers of single particles: irregular force, corrector) is
+    // written by a prediction pass only once a call has asked for it (or option "gather_copy" = 1)
+    bool gather_wanted = false, gather_valid = false;
+    int64_t opt_gather_copy = 0;
     // options
     int64_t opt_j_split = 0, opt_i_block = 0, opt_order_rows = 1, opt_irr_pred = 0, opt_fuse_pred = 1;
+    // fp64 fix-up of cancellation-dominated rows (fixflag.cuh): a row is recomputed iff C_a sqrt(q_a) > |acc| or
+    // C_j sqrt(q_j) > |jerk|; the options hold 1000 C_a and 1000 C_j
+    int64_t opt_fixup = 1, opt_fix_ca_milli = kFixCaMilli, opt_fix_cj_milli = kFixCjMilli;
     // last launch
     int64_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     // host path: device mirrors owned by the context
@@ -272,10 +298,12 @@ Plan make_plan(const Machine* c, int32_t n_i, int64_t opt_i_block, int64_t opt_j
     return best;
 }
 
-// two j-tile stages + their mbarriers + the fp64 running sums (6 per row, 7 with the potential)
-size_t force_smem_bytes(int ipt, int warps, int jt, bool pot) {
-    return 2 * (size_t)jt * kBytesPerJ + 2 * sizeof(uint64_t) +
-           (size_t)ipt * warps * 32 * (pot ? 7 : 6) * sizeof(double);
+// j-tile stages (two; one for the fused-prediction variant, PRED) + two mbarriers + the fp64 running sums (6 per row, 7
+// with the potential).
+// Per row also one float2 of error scales (fixflag.cuh).
+size_t force_smem_bytes(int ipt, int warps, int jt, bool pot, int stages = 2) {
+    return (size_t)stages * jt * kBytesPerJ + 2 * sizeof(uint64_t) +
+           (size_t)ipt * warps * 32 * ((pot ? 7 : 6) * sizeof(double) + sizeof(float2));
 }
 
 template <int IPT, int WARPS, int JT, int MINB, bool VEL, bool POT>
@@ -295,14 +323,20 @@ int launch_force(const Plan& p, const ForceArgs& fa, cudaStream_t st) {
     return NB_OK;
 }
 
-// The fused-prediction variant (force.cuh, PRED): plain criterion, no potential, shapes of 128 / 64 / 32 rows.
-int launch_force_pred(int shape, const Plan& p, const ForceArgs& fa, cudaStream_t st) {
-#define NB_PRED(WARPS, JT, MINB)                                                                      \
-    {                                                                                                 \
-        const size_t smem = force_smem_bytes(1, WARPS, JT, false); /* <= 27 KB: no opt-in needed */   \
-        force_kernel<1, WARPS, JT, MINB, false, false, true><<<p.grid, WARPS * 32, smem, st>>>(fa);   \
-        NB_CUDA(cudaGetLastError());                                                                  \
-        return NB_OK;                                                                                 \
+// The fused-prediction variant (force.cuh, PRED): plain criterion, no potential, shapes of 128 / 64 / 32 rows, one tile
+// stage.  per_sm != null: query the resident CTAs per SM instead of launching (the planner's slot count).
+int force_pred_dispatch(int shape, int* per_sm, const Plan* p, const ForceArgs* fa, cudaStream_t st) {
+#define NB_PRED(WARPS, JT, MINB)                                                                           \
+    {                                                                                                      \
+        auto kern = force_kernel<1, WARPS, JT, MINB, false, false, true>;                                  \
+        const size_t smem = force_smem_bytes(1, WARPS, JT, false, 1); /* <= 17 KB: no opt-in needed */     \
+        if (per_sm) {                                                                                      \
+            NB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, WARPS * 32, smem));        \
+            return NB_OK;                                                                                  \
+        }                                                                                                  \
+        kern<<<p->grid, WARPS * 32, smem, st>>>(*fa);                                                      \
+        NB_CUDA(cudaGetLastError());                                                                       \
+        return NB_OK;                                                                                      \
     }
     switch (shape) {
         case 1: NB_PRED(4, 256, NBREG_WARPS_PRED / 4)
@@ -339,7 +373,7 @@ int force_dispatch(int variant, int shape, int* per_sm, const Plan* p, const For
     }
 }
 
-int run_predict(nb_ctx* c, double t, cudaStream_t st, double* xp_out, double* vp_out) {
+int run_predict(nb_ctx* c, double t, cudaStream_t st, double* xp_out, double* vp_out, bool with_gather = false) {
     PredictArgs pa{};
     pa.n = c->n;
     pa.n_pairs = round_up(c->n, kJPad) / 2;
@@ -354,12 +388,23 @@ int run_predict(nb_ctx* c, double t, cudaStream_t st, double* xp_out, double* vp
     if (xp_out) {
         const int64_t pairs = (c->n + 1) / 2;
         pa.n_pairs = pairs;
-        predict_kernel<true><<<(unsigned)((pairs + threads - 1) / threads), threads, 0, st>>>(pa);
+        predict_kernel<true, false><<<(unsigned)((pairs + threads - 1) / threads), threads, 0, st>>>(pa);
+    } else if (with_gather) {
+        predict_kernel<false, true><<<(unsigned)((pa.n_pairs + threads - 1) / threads), threads, 0, st>>>(pa);
     } else {
-        predict_kernel<false><<<(unsigned)((pa.n_pairs + threads - 1) / threads), threads, 0, st>>>(pa);
+        predict_kernel<false, false><<<(unsigned)((pa.n_pairs + threads - 1) / threads), threads, 0, st>>>(pa);
     }
     NB_CUDA(cudaGetLastError());
     return NB_OK;
+}
+
+// The kernels that gather single particles (irregular force, corrector) read the particle-major copy of the predicted
+// records, which the predictor writes only on demand: make sure the context holds a prediction at t WITH that copy.
+// The first such call of a context sets gather_wanted, so that from then on every prediction pass writes it.
+int ensure_gather_prediction(nb_ctx* c, double t, void* stream) {
+    c->gather_wanted = true;
+    if (c->predicted && c->t_pred == t && c->gather_valid) return NB_OK;
+    return nb_predict_j(c, t, stream);
 }
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -431,6 +476,13 @@ int nb_create(nb_ctx** out, int device, int64_t n_max, int64_t n_i_max, int32_t 
             }
         }
     }
+    for (int k = 1; k <= 3; ++k) {
+        const int rc = force_pred_dispatch(k, &c->ctas_per_sm_pred[k], nullptr, nullptr, nullptr);
+        if (rc != NB_OK) {
+            delete c;
+            return rc;
+        }
+    }
     c->n_max = n_max;
     c->n_i_max = n_i_max;
     c->cap = nbr_cap;
@@ -486,6 +538,7 @@ int nb_set_j(nb_ctx* c, int64_t n, const double* x0, const double* v0, const dou
     c->n = n;
     c->x0 = x0; c->v0 = v0; c->a0 = a0; c->j0 = j0; c->m = m; c->t0 = t0;
     c->predicted = false;
+    c->gather_valid = false;
     return NB_OK;
 }
 
@@ -493,10 +546,12 @@ int nb_predict_j(nb_ctx* c, double t, void* stream) {
     if (!c) return NB_E_INVAL;
     if (c->n < 1) return NB_E_STATE;
     NB_CUDA(cudaSetDevice(c->device));
-    int rc = run_predict(c, t, static_cast<cudaStream_t>(stream), nullptr, nullptr);
+    const bool with_gather = c->gather_wanted || c->opt_gather_copy == 1;
+    int rc = run_predict(c, t, static_cast<cudaStream_t>(stream), nullptr, nullptr, with_gather);
     if (rc != NB_OK) return rc;
     c->predicted = true;
     c->t_pred = t;
+    c->gather_valid = with_gather;
     return NB_OK;
 }
 
@@ -537,7 +592,9 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         m0.n = c->n;
         m0.row_chunk_limit = c->lay.row_chunk_limit;
         m0.num_sms = c->num_sms;
-        for (int k = 0; k < kNumShapes; ++k) m0.ctas_per_sm[k] = c->ctas_per_sm[0][k];
+        // planned with the occupancy of the PRED instantiations (24 resident warps, not the 28 of the plain ones)
+        for (int k = 0; k < kNumShapes; ++k)
+            m0.ctas_per_sm[k] = (k >= 1 && k <= 3) ? c->ctas_per_sm_pred[k] : c->ctas_per_sm[0][k];
         const Plan p0 = make_plan(&m0, n_i, c->opt_i_block, c->opt_j_split);
         // one row block: every j predicted once.  A few row blocks: each predicts its j again, ~3 % more instructions
         // per block and 112 B/j of HBM reads that hide under the pair arithmetic, against a 38 us pass that nothing
@@ -561,7 +618,8 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     mach.row_chunk_limit = c->lay.row_chunk_limit;
     mach.num_sms = c->num_sms;
     const int variant = (dtr ? 1 : 0) | (pot ? 2 : 0);
-    for (int k = 0; k < kNumShapes; ++k) mach.ctas_per_sm[k] = c->ctas_per_sm[variant][k];
+    for (int k = 0; k < kNumShapes; ++k)
+        mach.ctas_per_sm[k] = (fuse_pred && k >= 1 && k <= 3) ? c->ctas_per_sm_pred[k] : c->ctas_per_sm[variant][k];
     const Plan p = make_plan(&mach, n_i, c->opt_i_block, c->opt_j_split);
     ForceArgs fa{};
     fa.raw = RawState{c->x0, c->v0, c->a0, c->j0, c->m, c->t0, t};
@@ -596,7 +654,7 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         OrderArgs oa{};
         oa.raw = fa.raw;
         oa.from_raw = fuse_pred;
-        oa.gather = reinterpret_cast<const float4*>(c->ws + c->lay.gather_off);
+        oa.packed = fa.packed;
         oa.i_idx = i_idx;
         oa.n_i = n_i;
         oa.box = reinterpret_cast<uint32_t*>(ctl + 4);
@@ -627,7 +685,17 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     }
     fa.slot_count = reinterpret_cast<int32_t*>(c->ws + c->lay.slot_off);
     fa.overflow_ws = ctl;
-    int rc = fuse_pred ? launch_force_pred(p.shape, p, fa, st) : force_dispatch(variant, p.shape, nullptr, &p, &fa, st);
+    fa.fix.count = ctl + 16;
+    fa.fix.rows = reinterpret_cast<int32_t*>(c->ws + c->lay.fixrow_off);
+    fa.fix.escale = reinterpret_cast<float2*>(c->ws + c->lay.escale_off);
+    {
+        const float ca = c->opt_fixup ? 1e-3f * (float)c->opt_fix_ca_milli : 0.f;
+        const float cj = c->opt_fixup ? 1e-3f * (float)c->opt_fix_cj_milli : 0.f;
+        fa.fix.ca2 = ca * ca;
+        fa.fix.cj2 = cj * cj;
+    }
+    int rc = fuse_pred ? force_pred_dispatch(p.shape, nullptr, &p, &fa, st)
+                       : force_dispatch(variant, p.shape, nullptr, &p, &fa, st);
     if (rc != NB_OK) return rc;
     ++launches;
     {  // S5 + n_overflow: always launched, with no rows when nothing was split
@@ -636,6 +704,7 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         ga.perm = fa.perm;
         ga.chunk_j = p.tiles_per_chunk * sh.jt;
         ga.part_sum = fa.part_sum;
+        ga.fix = fa.fix;
         ga.acc = acc; ga.jerk = jerk; ga.pot = pot; ga.nbr_count = nbr_count; ga.nbr_list = nbr_list; ga.n_overflow = n_overflow;
         ga.slot_count = fa.slot_count; ga.overflow_ws = ctl; ga.ticket = ctl + 1;
         const int64_t split_rows = has_split ? n_i - row0 : 0;
@@ -650,9 +719,27 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         NB_CUDA(cudaGetLastError());
         ++launches;
     }
+    if (c->opt_fixup) {  // fp64 fix-up of the rows the two kernels queued (usually none: every CTA returns at once)
+        FixupArgs xa{};
+        xa.raw = fa.raw;
+        xa.n = (int32_t)c->n;
+        xa.i_idx = i_idx; xa.r_s = r_s; xa.dtr = dtr;
+        xa.acc = acc; xa.jerk = jerk;
+        xa.count = fa.fix.count; xa.rows = fa.fix.rows;
+        xa.part = fa.part_sum;
+        xa.tickets = reinterpret_cast<int32_t*>(c->ws + c->lay.ftick_off);
+        xa.done = ctl + 17;
+        xa.stat_last = ctl + 18;
+        xa.stat_total = reinterpret_cast<unsigned long long*>(ctl + 20);
+        const unsigned grid = (unsigned)std::min(kFixMaxGrid, 2 * c->num_sms);
+        if (dtr) fixup_kernel<true><<<grid, kFixThreads, 0, st>>>(xa);
+        else fixup_kernel<false><<<grid, kFixThreads, 0, st>>>(xa);
+        NB_CUDA(cudaGetLastError());
+        ++launches;
+    }
     c->info[0] = sh.rows; c->info[1] = sh.ipt; c->info[2] = p.n_chunks; c->info[3] = p.grid;
     c->info[4] = p.n_blocks - p.main_blocks; c->info[5] = launches; c->info[6] = sh.jt;
-    c->info[7] = c->ctas_per_sm[variant][p.shape];
+    c->info[7] = mach.ctas_per_sm[p.shape];
     return NB_OK;
 }
 
@@ -668,8 +755,8 @@ int irregular_launch(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const int32_t
     if (c->n < 1) return NB_E_STATE;
     NB_CUDA(cudaSetDevice(c->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (!act && (!c->predicted || c->t_pred != t)) {  // predict all particles first, same stream (PRED_ALL)
-        int rc = nb_predict_j(c, t, stream);
+    if (!act) {  // predict all particles first, same stream (PRED_ALL), unless the context already holds them
+        int rc = ensure_gather_prediction(c, t, stream);
         if (rc != NB_OK) return rc;
     }
     if (n_i == 0) return NB_OK;
@@ -696,7 +783,7 @@ int nb_irregular_force(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const int32
     // The paper's switch between PRED_ALL and PRED_ACT (NPACT of Listing C1): with no prediction at t in
     // the context, a block of at most n / kIrrActRatio rows predicts what it gathers (measured turn-around: ~3000 rows
     // at n = 65536, ~10000 at n = 2^20).  Both modes return the same bits.
-    const bool stale = c && (!c->predicted || c->t_pred != t);
+    const bool stale = c && (!c->predicted || c->t_pred != t || !c->gather_valid);
     const bool act = c && (c->opt_irr_pred == 2 ||
                            (c->opt_irr_pred == 0 && stale && (int64_t)n_i * kIrrActRatio <= c->n));
     return irregular_launch(c, n_i, i_idx, nbr_count, nbr_list, list_stride, t, acc, jerk, stream, act);
@@ -720,10 +807,10 @@ int nb_regular_correct(nb_ctx* c, int32_t n_i, const nb_corrector_io* io, double
     NB_CUDA(cudaSetDevice(c->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     // as nb_irregular_force: a small block without a prediction at t predicts what it gathers ("irr_pred")
-    const bool stale = !c->predicted || c->t_pred != t;
+    const bool stale = !c->predicted || c->t_pred != t || !c->gather_valid;
     const bool act = c->opt_irr_pred == 2 || (c->opt_irr_pred == 0 && stale && (int64_t)n_i * kIrrActRatio <= c->n);
-    if (stale && !act) {
-        int rc = nb_predict_j(c, t, stream);
+    if (!act) {
+        int rc = ensure_gather_prediction(c, t, stream);
         if (rc != NB_OK) return rc;
     }
     if (n_i == 0) return NB_OK;
@@ -746,10 +833,28 @@ int nb_regular_correct(nb_ctx* c, int32_t n_i, const nb_corrector_io* io, double
     return NB_OK;
 }
 
+static int regular_force_host_impl(nb_ctx* c, int64_t n, const double* x0, const double* v0, const double* a0,
+                                   const double* j0, const double* m, const double* t0, int32_t n_i,
+                                   const int32_t* i_idx, const double* r_s, double t, double* acc, double* jerk,
+                                   int32_t* nbr_count, int32_t* nbr_list, int32_t* n_overflow);
+
 int nb_regular_force_host(nb_ctx* c, int64_t n, const double* x0, const double* v0, const double* a0,
                           const double* j0, const double* m, const double* t0, int32_t n_i, const int32_t* i_idx,
                           const double* r_s, double t, double* acc, double* jerk, int32_t* nbr_count,
                           int32_t* nbr_list, int32_t* n_overflow) {
+    const int rc = regular_force_host_impl(c, n, x0, v0, a0, j0, m, t0, n_i, i_idx, r_s, t, acc, jerk, nbr_count,
+                                           nbr_list, n_overflow);
+    if (rc != NB_OK && c) {  // leave nothing of this call in flight: the caller may free or reuse its host buffers
+        if (c->hstream) cudaStreamSynchronize(c->hstream);
+        if (c->hcopy) cudaStreamSynchronize(c->hcopy);
+    }
+    return rc;
+}
+
+static int regular_force_host_impl(nb_ctx* c, int64_t n, const double* x0, const double* v0, const double* a0,
+                                   const double* j0, const double* m, const double* t0, int32_t n_i,
+                                   const int32_t* i_idx, const double* r_s, double t, double* acc, double* jerk,
+                                   int32_t* nbr_count, int32_t* nbr_list, int32_t* n_overflow) {
     if (!c || !x0 || !v0 || !a0 || !j0 || !m || !t0 || !n_overflow) return NB_E_INVAL;
     if (n < 1 || n > c->n_max || n_i < 0 || n_i > c->n_i_max) return NB_E_INVAL;
     if (n_i > 0 && (!i_idx || !r_s || !acc || !jerk || !nbr_count || !nbr_list)) return NB_E_INVAL;
@@ -842,6 +947,29 @@ int nb_regular_force_host(nb_ctx* c, int64_t n, const double* x0, const double* 
     return NB_OK;
 }
 
+int nb_get_error_scale(nb_ctx* c, int32_t n_i, float* escale, void* stream) {
+    if (!c || n_i < 0 || n_i > c->n_i_max || (n_i > 0 && !escale)) return NB_E_INVAL;
+    NB_CUDA(cudaSetDevice(c->device));
+    if (n_i > 0)
+        NB_CUDA(cudaMemcpyAsync(escale, c->ws + c->lay.escale_off, (size_t)n_i * sizeof(float2),
+                                cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(stream)));
+    return NB_OK;
+}
+
+int nb_fixup_stats(nb_ctx* c, int64_t stats[2], void* stream) {
+    if (!c || !stats) return NB_E_INVAL;
+    NB_CUDA(cudaSetDevice(c->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int32_t h[4] = {0, 0, 0, 0};
+    NB_CUDA(cudaMemcpyAsync(h, c->ws + c->lay.ctl_off + 18 * sizeof(int32_t), sizeof(h), cudaMemcpyDeviceToHost, st));
+    NB_CUDA(cudaStreamSynchronize(st));
+    unsigned long long total;
+    memcpy(&total, h + 2, sizeof(total));
+    stats[0] = h[0];
+    stats[1] = (int64_t)total;
+    return NB_OK;
+}
+
 int nb_set_option(nb_ctx* c, const char* key, int64_t value) {
     if (!c || !key || value < 0) return NB_E_INVAL;
     if (!strcmp(key, "j_split")) {
@@ -856,6 +984,24 @@ int nb_set_option(nb_ctx* c, const char* key, int64_t value) {
     if (!strcmp(key, "fuse_pred")) {
         if (value > 2) return NB_E_INVAL;
         c->opt_fuse_pred = value;
+        return NB_OK;
+    }
+    if (!strcmp(key, "gather_copy")) {
+        if (value > 1) return NB_E_INVAL;
+        c->opt_gather_copy = value;
+        return NB_OK;
+    }
+    if (!strcmp(key, "fixup")) {
+        if (value > 1) return NB_E_INVAL;
+        c->opt_fixup = value;
+        return NB_OK;
+    }
+    if (!strcmp(key, "fixup_ca_milli")) {
+        c->opt_fix_ca_milli = value;
+        return NB_OK;
+    }
+    if (!strcmp(key, "fixup_cj_milli")) {
+        c->opt_fix_cj_milli = value;
         return NB_OK;
     }
     if (!strcmp(key, "irr_pred")) {

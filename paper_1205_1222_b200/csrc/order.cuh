@@ -31,7 +31,7 @@ constexpr int kOrderThreads = 256;
 struct OrderArgs {
     RawState raw;           // from_raw: the registered fp64 state and the time to predict to
     bool from_raw;          // the context holds no prediction (fused-prediction call): predict the rows' positions here
-    const float4* gather;   // particle-major predicted records
+    const float4* packed;   // pair-interleaved predicted records (nbreg_common.cuh)
     const int32_t* i_idx;   // [n_i]
     int32_t n_i;
     uint32_t* box;          // [6] order-preserving images: max of x, y, z and max of the complemented images (= min)
@@ -68,8 +68,10 @@ __device__ __forceinline__ float3 row_position(const OrderArgs& a, int32_t q) {
         const PredRecord r = predict_record(a.raw, a.i_idx[q]);
         return make_float3(r.xh, r.yh, r.zh);
     }
-    const float4 g0 = __ldg(a.gather + (size_t)a.i_idx[q] * kGatherQuads);
-    return make_float3(g0.x, g0.y, g0.z);
+    // the high words of particle i in its pair record: { xh0, xh1, yh0, yh1 } { zh0, zh1, .. }
+    const int32_t i = a.i_idx[q];
+    const float* rec = reinterpret_cast<const float*>(a.packed + (size_t)(i >> 1) * kQuadsPerPair) + (i & 1);
+    return make_float3(__ldg(rec), __ldg(rec + 2), __ldg(rec + 4));
 }
 __device__ __forceinline__ void box_scale(const uint32_t box[6], float lo[3], float scale[3]) {
 #pragma unroll

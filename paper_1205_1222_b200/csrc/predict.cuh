@@ -1,8 +1,11 @@
 // predict.cuh -- S1, the Hermite j-predictor (step (iii) "Predict all particles"; the paper runs it
 // on the host as CXVPRED, and prints no formula: BASELINE.json north_star fixes
 //   x_p = x0 + v0 dt + a0 dt^2/2 + j0 dt^3/6,   v_p = v0 + a0 dt + j0 dt^2/2,   dt = t - t0[j]).
-// HBM-bound: reads 112 B and writes 40 B per particle.  One thread per PAIR of particles so that every
-// global access is a 16-byte vector: 3 x double2 per [2][3] block of each state array, 5 x float4 out.
+// HBM-bound: reads 112 B and writes 40 B per particle (SURVEY 8(a) S1 budgets 112 + 48).  One thread per PAIR of
+// particles so that every global access is a 16-byte vector: 3 x double2 per [2][3] block of each state array,
+// 5 x float4 out.  The particle-major copy for the kernels that gather single particles (irregular.cuh, corrector.cuh;
+// 48 B per particle more) is written only when such a consumer exists (GATHER): the regular-force path alone never
+// pays for it.
 #pragma once
 #include "nbreg_common.cuh"
 
@@ -19,7 +22,7 @@ struct PredictArgs {
     const double* t0;
     double t;
     float4* packed;
-    float4* gather;    // [n][3] particle-major copy of the predicted records (nbreg_common.cuh)
+    float4* gather;    // GATHER: [n][3] particle-major copy of the predicted records (nbreg_common.cuh)
     float* tile_vmax;  // [n_pad / 256] upper bound of |v_p| over each block of 256 consecutive particles
     double* xp_out;  // fp64 outputs (test hook), used only when WRITE_F64
     double* vp_out;
@@ -40,7 +43,7 @@ __device__ __forceinline__ void load3(const double* base, int64_t j, double (&ou
 // The kernel also leaves, per block of 256 consecutive particles (= kJPad, a multiple of every j-tile), an upper
 // bound of the predicted speed: the velocity neighbour criterion eq. (3) needs |V_ij| bounded to
 // decide that a far pair cannot come within r_s during dtr (force.cuh).
-template <bool WRITE_F64>
+template <bool WRITE_F64, bool GATHER>
 __global__ void __launch_bounds__(256) predict_kernel(PredictArgs a) {
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool active = p < a.n_pairs;
@@ -117,7 +120,7 @@ __global__ void __launch_bounds__(256) predict_kernel(PredictArgs a) {
         o[2] = make_float4(vf[0], vf[3], vf[1], vf[4]);
         o[3] = make_float4(vf[2], vf[5], xl[0], xl[3]);
         o[4] = make_float4(xl[1], xl[4], xl[2], xl[5]);
-        if (j0 < a.n) {  // particle-major copy: the pair's two records are contiguous (96 B)
+        if (GATHER && j0 < a.n) {  // particle-major copy: the pair's two records are contiguous (96 B)
             float4* g = a.gather + kGatherQuads * j0;
             g[0] = make_float4(xh[0], xh[1], xh[2], mf[0]);
             g[1] = make_float4(xl[0], xl[1], xl[2], vf[0]);

@@ -30,6 +30,7 @@ def run_gpu(wl, options=None, n_max=None, n_i_max=None, cap=None, ctx=None, want
         ctx.nb_regular_force_ex(i_idx, r_s, s.t, dtr=dtr_t, want_pot=want_pot, out=out)
     torch.cuda.synchronize()
     info = ctx.nb_last_launch_info()
+    info["fixup_rows"] = ctx.nb_fixup_stats()["last"]  # rows the call recomputed in fp64 (fixup.cuh)
     gpu = {k: v.cpu().numpy() for k, v in out.items()}
     res = [gpu, info]
     if want_pred:

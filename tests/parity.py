@@ -44,10 +44,15 @@ def _pair_terms(xp, vp, m, i, js):
     return da, dj, float((m[js] / r).sum())
 
 
-def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None, dtr=None, check_pot=False):
+def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None, dtr=None, check_pot=False,
+            precomputed=None, strict=True):
     """gpu: dict of numpy arrays acc, jerk, nbr_count, nbr_list, n_overflow (full block).
     rows: optional subset of row numbers to check (oracle runs only on those).
     dtr: per-row regular steps -> velocity criterion eq. (3) (band measured on r_min); check_pot: compare gpu["pot"].
+    precomputed: (acc, jerk, count, lists) of oracle.regular_force on exactly these rows (bench.py times that call as
+    its cpu_baseline and hands the results in, so the oracle runs once).
+    strict=False: rows over the acc / jerk tolerance are counted (rows_over_acc, rows_over_jerk) instead of raising
+    (list violations still raise): for measuring how many rows the fp32 path alone would miss.
     Returns a report dict; raises AssertionError on a violation."""
     i_idx = np.asarray(i_idx)
     if rows is None:
@@ -58,7 +63,11 @@ def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None
     stride = list_stride or max(2 * cap, 64)
     ex = dtr is not None or check_pot
     sub_dt = np.zeros(rows.shape[0]) if dtr is None else np.ascontiguousarray(np.asarray(dtr)[rows], dtype=np.float64)
-    if ex:
+    if precomputed is not None:
+        assert not ex
+        acc_o, jerk_o, cnt_o, lists_o = (np.array(precomputed[0]), np.array(precomputed[1]), precomputed[2],
+                                         precomputed[3])
+    elif ex:
         acc_o, jerk_o, pot_o, cnt_o, lists_o = oracle.regular_force_ex(xp, vp, m, sub_idx, sub_rs,
                                                                        None if dtr is None else sub_dt, list_stride=stride)
     else:
@@ -66,7 +75,7 @@ def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None
     acc_g, jerk_g = gpu["acc"][rows].copy(), gpu["jerk"][rows].copy()
     cnt_g = gpu["nbr_count"][rows]
     list_g = gpu["nbr_list"][rows]
-    n_band_pairs, worst_band, n_over = 0, 0.0, 0
+    n_band_pairs, worst_band, n_over, n_bestfit = 0, 0.0, 0, 0
     recheck = []  # rows whose list differs only inside the band
     for q in range(rows.shape[0]):
         so = lists_o[q]
@@ -110,6 +119,10 @@ def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None
             assert abs(delta) <= len(cand), f"row {rows[q]}: overflow count mismatch"
             best = None
             if delta != 0:
+                # The only place where the harness fits something to the output under test: WHICH band pairs of an
+                # overflowed row were left out of the stored list cannot be read off the list.  Counted and reported
+                # (overflow_bestfit); 0 on configs 1-5.
+                n_bestfit += 1
                 for combo in itertools.islice(itertools.combinations(cand, abs(delta)), 256):
                     da, dj, dp = _pair_terms(xp, vp, m, i, np.array(combo))
                     sign = 1.0 if delta > 0 else -1.0
@@ -149,8 +162,9 @@ def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None
     if zero.any():
         assert np.all(acc_g[zero] == 0) and np.all(jerk_g[zero] == 0)
     worst_a = int(np.argmax(ea))
-    assert ea.max() <= TOL_ACC, f"acc rel err {ea.max():.3e} at row {rows[worst_a]} > {TOL_ACC}"
-    assert ej.max() <= TOL_JERK, f"jerk rel err {ej.max():.3e} at row {rows[int(np.argmax(ej))]} > {TOL_JERK}"
+    if strict:
+        assert ea.max() <= TOL_ACC, f"acc rel err {ea.max():.3e} at row {rows[worst_a]} > {TOL_ACC}"
+        assert ej.max() <= TOL_JERK, f"jerk rel err {ej.max():.3e} at row {rows[int(np.argmax(ej))]} > {TOL_JERK}"
     max_pot = 0.0
     if check_pot:
         pot_g = gpu["pot"][rows]
@@ -162,7 +176,10 @@ def compare(oracle, xp, vp, m, i_idx, r_s, cap, gpu, rows=None, list_stride=None
         max_pot = float(ep.max())
     return dict(max_pot_err=max_pot, rows=int(rows.shape[0]), max_acc_err=float(ea.max()), max_jerk_err=float(ej.max()),
                 median_acc_err=float(np.median(ea)), band_pairs=int(n_band_pairs), worst_band=float(worst_band),
-                overflow_rows=int(n_over), mean_count=float(cnt_o.mean()))
+                overflow_rows=int(n_over), overflow_bestfit=int(n_bestfit), mean_count=float(cnt_o.mean()),
+                p999_jerk_err=float(np.quantile(ej, 0.999)) if len(ej) else 0.0,
+                rows_over_half_tol=int(((ea > 0.5 * TOL_ACC) | (ej > 0.5 * TOL_JERK)).sum()),
+                rows_over_acc=int((ea > TOL_ACC).sum()), rows_over_jerk=int((ej > TOL_JERK).sum()))
 
 
 def check_overflow_flag(gpu, cap):

@@ -44,10 +44,13 @@ def _check_irregular(oracle, xp, vp, m, i_idx, out, cap, rows=None):
     ea, ej = da[ok] / sa[ok], dj[ok] / sj[ok]
     assert ea.max() <= TOL_TERMS, f"acc: {ea.max():.3e} of the summed term norms"
     assert ej.max() <= TOL_TERMS, f"jerk: {ej.max():.3e} of the summed term norms"
+    # the same deviations relative to the result itself: a loosened yardstick (pinned: tests/test_oracle_pins.py P13)
+    # would show here
     rel_a = da[ok] / np.linalg.norm(a_o[ok], axis=1)
+    rel_j = dj[ok] / np.linalg.norm(j_o[ok], axis=1)
+    q = lambda r: dict(median=float(np.median(r)), p99=float(np.quantile(r, 0.99)), max=float(r.max()))
     return dict(rows=int(len(rows)), max_err_vs_terms=(float(ea.max()), float(ej.max())),
-                acc_rel_to_result=dict(median=float(np.median(rel_a)), p99=float(np.quantile(rel_a, 0.99)),
-                                       max=float(rel_a.max())))
+                acc_rel_to_result=q(rel_a), jerk_rel_to_result=q(rel_j))
 
 
 @pytest.mark.parametrize("config", [1, 2, 4])

@@ -381,6 +381,39 @@ def test_irregular_two_body_and_ring(impl):
     assert np.all(res[0] == 0) and np.all(res[1] == 0)
 
 
+def test_p13_irregular_scales_closed_form():
+    """The yardstick itself: acc_scale = sum m_j / r^2 and jerk_scale = sum 4 m_j |V_ij| / r^3 of eq. (7), (8)
+     are the tolerance of the NEXT-2 / NEXT-4 GPU tests, so they are pinned to hand-derived values
+    (tests/golden/closed_forms.json P13): a scale 10 x too large would loosen three GPU test families unnoticed."""
+    g, gs = GOLD["P1_two_body"], GOLD["P13_irregular_scales"]
+    xp = np.array([g["xi"], g["xj"]], dtype=float)
+    vp = np.array([g["vi"], g["vj"]], dtype=float)
+    m = np.array([7.0, g["mj"]])  # m_i must not enter
+    _, _, sa, sj = oracle.irregular_force(xp, vp, m, np.array([0], dtype=np.int32), [np.array([1, 0], dtype=np.int32)])
+    assert abs(sa[0] - gs["two_body_acc_scale"]) < 1e-17 and abs(sj[0] - gs["two_body_jerk_scale"]) < 1e-17
+    # twice the mass, twice the scales; an empty list has none
+    _, _, sa2, sj2 = oracle.irregular_force(xp, vp, np.array([7.0, 2 * g["mj"]]), np.array([0], dtype=np.int32),
+                                            [np.array([1], dtype=np.int32)])
+    assert abs(sa2[0] - 2 * gs["two_body_acc_scale"]) < 1e-16 and abs(sj2[0] - 2 * gs["two_body_jerk_scale"]) < 1e-16
+    _, _, sa0, sj0 = oracle.irregular_force(xp, vp, m, np.array([0], dtype=np.int32), [np.array([], dtype=np.int32)])
+    assert sa0[0] == 0.0 and sj0[0] == 0.0
+    # the ring of P2 as the list of the particle on the axis
+    r = GOLD["P2_ring"]
+    nr = r["n_ring"]
+    ang = 2 * np.pi * np.arange(nr) / nr
+    xp = np.zeros((nr + 1, 3))
+    xp[:nr, 0] = r["radius"] * np.cos(ang)
+    xp[:nr, 1] = r["radius"] * np.sin(ang)
+    xp[nr] = [0, 0, r["zi"]]
+    vp = np.zeros((nr + 1, 3))
+    vp[nr] = [0, 0, r["wi"]]
+    m = np.full(nr + 1, r["m_each"])
+    a, j, sa, sj = oracle.irregular_force(xp, vp, m, np.array([nr], dtype=np.int32), [np.arange(nr, dtype=np.int32)])
+    assert abs(sa[0] - gs["ring_acc_scale"]) < 1e-16 and abs(sj[0] - gs["ring_jerk_scale"]) < 1e-16
+    np.testing.assert_allclose(a[0], r["acc"], atol=1e-16)  # the list sum of everybody = the regular sum with r_s = 0
+    np.testing.assert_allclose(j[0], r["jerk"], atol=1e-16)
+
+
 def test_irregular_plus_regular_is_total():
     """eq. (7) + eq. (9) = total force, eq. (8) + eq. (10) = total jerk, for any r_s: the list
     sum and the masked all-j sum are two different loops of the oracle."""
