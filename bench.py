@@ -35,6 +35,12 @@ LANE_SLOTS_PER_PAIR = 25.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE force_kernel launch of the default workload, from the
 # committed capture profiles/r1_force_kernel_c5_ncu_full.md (ncu --set full); None for other workloads.
 FORCE_DRAM_BYTES_C5 = 1262.53e6 + 790.06e6
+# algorithmic bytes of the predictor per particle on the regular-force path: 112 B of fp64 state read, 40 B of
+# pair-interleaved record written (the 48 B particle-major copy is written only for gathering consumers)
+PRED_BYTES_PER_J = 152
+# dram__bytes_read.sum + dram__bytes_write.sum of one predict_kernel launch of the default workload (ncu --set full,
+# profiles/r2_predict_kernel_c5_ncu_full.md); None until captured
+PRED_DRAM_BYTES_C5 = None
 METRIC = "regular-force Ginteractions/s (acc+jerk+nbr list)"
 UNIT = "Gpairs/s"
 
@@ -104,14 +110,57 @@ def whole_job_rate(pairs_per_rank_step: int, steps: int, world: int, t_max_secon
     return world * pairs_per_rank_step * steps / t_max_seconds / 1e9
 
 
+def shard_job(wl, rank: int, world: int, mode: str):
+    """What one rank runs and how the job is counted.  mode "none": every rank runs the whole workload (N independent
+    replicas: the job is `world` times the workload's pairs).  mode "rows": ONE job, its rows split over
+    the ranks on CTA boundaries, no data-path collective (strong scaling: the job is the workload's pairs once).
+    Returns (this rank's workload, pairs of ONE replica or of the whole job, replicas, this rank's rows or None)."""
+    if mode != "rows":
+        return wl, wl.pairs, world, None
+    import dataclasses
+    from paper_1205_1222_b200 import sharding
+    lo, hi = sharding.row_shard(wl.n_i, rank, world)
+    local = dataclasses.replace(wl, i_idx=np.ascontiguousarray(wl.i_idx[lo:hi]), r_s=np.ascontiguousarray(wl.r_s[lo:hi]))
+    return local, wl.pairs, 1, (lo, hi)
+
+
 def build_workload(config: int, n_i: int | None):
     from paper_1205_1222_b200 import inputs
     wl = inputs.make_workload(config, n_i=n_i)
     return wl
 
 
-def cpu_baseline(wl, target_seconds: float = 12.0, steps: int = 1):
-    """The oracle as it stands, on this host's cores, on a bounded sample of rows of the same workload."""
+def cpu_description() -> dict:
+    """CPU model, logical CPUs, physical cores and whether SMT siblings are counted."""
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    logical = os.cpu_count() or 0
+    physical = None
+    try:
+        import psutil
+        physical = psutil.cpu_count(logical=False)
+    except Exception:
+        pass
+    try:
+        affinity = len(os.sched_getaffinity(0))
+    except Exception:
+        affinity = logical
+    smt = None if not physical else (logical > physical)
+    return {"cpu_model": model, "logical_cpus": logical, "physical_cores": physical, "usable_cpus": affinity,
+            "smt": ("on: OpenMP threads land on SMT siblings too" if smt else "off or not visible") if smt is not None
+                   else "unknown"}
+
+
+def cpu_baseline(wl, target_seconds: float = 12.0, steps: int = 1, min_rows: int = 0, single_thread: bool = True):
+    """The oracle as it stands, on this host's cores, on a bounded sample of rows of the same workload (the first
+    `rows` active rows against all j).  Returns (report, seconds per pass, rows, oracle results of those rows): the
+    results double as the reference of the in-run parity check, so the oracle runs once."""
     from oracle import oracle
     s = wl.state
     xp, vp = oracle.predict_state(s)
@@ -121,17 +170,48 @@ def cpu_baseline(wl, target_seconds: float = 12.0, steps: int = 1):
     oracle.regular_force(xp, vp, s.m, wl.i_idx[:rows], wl.r_s[:rows], list_stride=2 * wl.cap)
     dt = time.perf_counter() - t0
     rate = rows * s.n / dt
-    rows = int(min(wl.n_i, max(rows, rate * target_seconds / s.n)))
+    rows = int(min(wl.n_i, max(rows, min_rows, rate * target_seconds / s.n)))
     rows = max(cores, rows // cores * cores)
     rows = min(rows, wl.n_i)
-    times = []
+    times, res = [], None
     for _ in range(steps):
         t0 = time.perf_counter()
-        oracle.regular_force(xp, vp, s.m, wl.i_idx[:rows], wl.r_s[:rows], list_stride=2 * wl.cap)
+        res = oracle.regular_force(xp, vp, s.m, wl.i_idx[:rows], wl.r_s[:rows], list_stride=2 * wl.cap)
         times.append(time.perf_counter() - t0)
     dt = float(np.mean(times))
-    return dict(value=rows * s.n / dt / 1e9, unit=UNIT, cores=cores, kind="oracle",
-                sample=f"first {rows} active rows x all {s.n} j (fp64, OpenMP, gcc -O2), {dt:.2f} s per pass"), dt
+    rep = dict(value=rows * s.n / dt / 1e9, unit=UNIT, cores=cores, kind="oracle",
+               sample=f"first {rows} active rows x all {s.n} j (fp64, OpenMP, gcc -O2), {dt:.2f} s per pass")
+    rep.update(cpu_description())
+    if single_thread:  # one thread, fewer rows (about a second of work)
+        r1 = int(max(4, min(rows, rate / max(cores, 1) * 1.0 / s.n)))
+        oracle.set_num_threads(1)
+        t0 = time.perf_counter()
+        oracle.regular_force(xp, vp, s.m, wl.i_idx[:r1], wl.r_s[:r1], list_stride=2 * wl.cap)
+        t1 = time.perf_counter() - t0
+        oracle.set_num_threads(cores)
+        rep["single_thread"] = {"value": r1 * s.n / t1 / 1e9, "unit": UNIT, "sample": f"first {r1} rows, {t1:.2f} s"}
+    return rep, dt, rows, (res, xp, vp)
+
+
+def parity_in_run(wl, out, rows, oracle_results) -> dict:
+    """parity checked in the same run, on the outputs of the last timed repetition, against the oracle
+    results the cpu_baseline leg has just computed for the first `rows` rows (north_star's tolerances, tests/parity.py)."""
+    tests_dir = os.path.join(ROOT, "tests")
+    if tests_dir not in sys.path:
+        sys.path.insert(0, tests_dir)
+    import parity
+    from oracle import oracle
+    (acc_o, jerk_o, cnt_o, lists_o), xp, vp = oracle_results
+    gpu = {k: v[:rows].cpu().numpy() if k != "n_overflow" else v.cpu().numpy() for k, v in out.items()}
+    s = wl.state
+    try:
+        rep = parity.compare(oracle, xp, vp, s.m, wl.i_idx[:rows], wl.r_s[:rows], wl.cap, gpu,
+                             precomputed=(acc_o, jerk_o, cnt_o, lists_o))
+        return {"ok": True, "rows": rep["rows"], "max_acc": rep["max_acc_err"], "max_jerk": rep["max_jerk_err"],
+                "band_pairs": rep["band_pairs"], "overflow_rows": rep["overflow_rows"],
+                "tolerance": {"acc": parity.TOL_ACC, "jerk": parity.TOL_JERK, "band": parity.BAND}}
+    except AssertionError as e:
+        return {"ok": False, "rows": int(rows), "error": str(e)[:300]}
 
 
 def run_reference(args):
@@ -140,8 +220,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     wl = build_workload(args.config, args.n_i)
-    base, _ = cpu_baseline(wl, target_seconds=4.0, steps=1)  # sizes the sample
-    rows = int(base["sample"].split()[1])
+    base, _, rows, _ = cpu_baseline(wl, target_seconds=4.0, steps=1, single_thread=False)  # sizes the sample
     from oracle import oracle
     s = wl.state
     xp, vp = oracle.predict_state(s)
@@ -155,6 +234,7 @@ def run_reference(args):
     val = rows * s.n / dt / 1e9
     cb = dict(value=val, unit=UNIT, cores=base["cores"], kind="oracle",
               sample=f"each step: predictor on all {s.n} + first {rows} active rows x all j")
+    cb.update(cpu_description())
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
@@ -267,9 +347,89 @@ def run_sweep(args):
     return 0
 
 
+class Bench:
+    """One workload resident on one GPU: context, device inputs, outputs, and the timed step."""
+
+    def __init__(self, wl, local: int):
+        import torch
+        from paper_1205_1222_b200 import binding
+        self.torch, self.wl, self.s = torch, wl, wl.state
+        self.dev = torch.device(f"cuda:{local}")
+        self.ctx = binding.Context(self.s.n, wl.n_i, wl.cap, device=local)
+        self.state_dev = self.ctx.set_state(self.s)
+        self.i_idx = torch.from_numpy(wl.i_idx).to(self.dev)
+        self.r_s = torch.from_numpy(wl.r_s).to(self.dev)
+        self.out = self.ctx.alloc_outputs(wl.n_i)
+
+    def step(self, ev=None):
+        """One pass of the whole hot path: nb_set_j -> nb_predict_j (S1) -> nb_regular_force (S2-S6 + fix-up)."""
+        self.ctx.nb_set_j(*self.state_dev)     # GPUNB_SEND: new block-step, prediction invalid
+        if ev: ev[0].record()
+        self.ctx.nb_predict_j(self.s.t)        # S1
+        if ev: ev[1].record()
+        self.ctx.nb_regular_force(self.i_idx, self.r_s, self.s.t, out=self.out)  # prediction already at t
+        if ev: ev[2].record()
+
+    def timed(self, steps: int, warmup: int, flush, dist=None):
+        """W warm-up steps, then K steps, each bracketed by CUDA events on the launching stream; the L2 flush between
+        steps sits outside the events.  Returns per-step seconds (step, predictor, force) and the launch info."""
+        torch = self.torch
+        for _ in range(max(warmup, 3)):
+            self.step()
+        torch.cuda.synchronize()
+        info = self.ctx.nb_last_launch_info()
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+        if dist: dist.barrier()
+        torch.cuda.synchronize()
+        for k in range(steps):
+            flush.fill_(k & 0xff)              # L2 flush between timed iterations (outside the per-step events)
+            self.step(evs[k])
+        torch.cuda.synchronize()
+        if dist: dist.barrier()
+        t_step = np.array([e[0].elapsed_time(e[2]) for e in evs]) / 1e3
+        t_pred = np.array([e[0].elapsed_time(e[1]) for e in evs]) / 1e3
+        t_force = np.array([e[1].elapsed_time(e[2]) for e in evs]) / 1e3
+        info["fixup_rows"] = self.ctx.nb_fixup_stats()["last"]
+        return t_step, t_pred, t_force, info
+
+    def close(self):
+        self.ctx.close()
+
+
+def fp32_peak_tflops(torch, local, peaks):
+    nsm = torch.cuda.get_device_properties(local).multi_processor_count
+    return nsm, nsm * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+
+
+def run_also(config: int, local: int, flush, peaks, steps: int) -> dict:
+    """The other configs of BASELINE.json beside the headline: the same step, the same event protocol, clocks sampled
+    during the timed region, and parity of the last timed repetition against the oracle on >= 1024 seeded rows."""
+    import torch
+    wl = build_workload(config, None)
+    b = Bench(wl, local)
+    sampler = ClockSampler(local)
+    sampler.start()
+    t_step, t_pred, t_force, info = b.timed(steps, 3, flush)
+    clocks = sampler.stop()
+    nsm, peak_tf = fp32_peak_tflops(torch, local, peaks)
+    cb, _, rows, ores = cpu_baseline(wl, target_seconds=1.0, min_rows=min(wl.n_i, 1024), single_thread=False)
+    par = parity_in_run(wl, b.out, rows, ores)
+    med = float(np.median(t_step))
+    res = {"config": config, "workload": f"N={wl.state.n}, N_i={wl.n_i}, k~{wl.k}, cap {wl.cap}",
+           "value": wl.pairs / float(np.mean(t_step)) / 1e9, "unit": UNIT,
+           "value_median": wl.pairs / med / 1e9, "value_best": wl.pairs / float(t_step.min()) / 1e9,
+           "us_per_step": float(np.mean(t_step)) * 1e6, "us_force_call": float(np.mean(t_force)) * 1e6,
+           "us_predictor": float(np.mean(t_pred)) * 1e6, "steps": steps,
+           "frac": wl.pairs * FLOPS_PER_PAIR / float(np.mean(t_force)) / 1e12 / peak_tf,
+           "frac_whole_step": wl.pairs * FLOPS_PER_PAIR / float(np.mean(t_step)) / 1e12 / peak_tf,
+           "launch": info, "clocks": clocks, "parity": par,
+           "cpu_baseline": {"value": cb["value"], "unit": UNIT, "cores": cb["cores"], "sample": cb["sample"]}}
+    b.close()
+    return res
+
+
 def run_gpu_arm(args):
     import torch
-    from paper_1205_1222_b200 import binding
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -284,49 +444,19 @@ def run_gpu_arm(args):
     dev = torch.device(f"cuda:{local}")
     peaks = _peaks()
     wl = build_workload(args.config, args.n_i)  # every rank: the same seeded workload (independent replicas)
-    job_pairs, job_replicas, shard_rows = wl.pairs, world, None
-    if args.shard == "rows":  # ONE job, its rows split over the ranks (strong scaling); no data-path collective
-        import dataclasses
-        from paper_1205_1222_b200 import sharding
-        shard_rows = sharding.row_shard(wl.n_i, rank, world)
-        job_replicas = 1
-        wl = dataclasses.replace(wl, i_idx=np.ascontiguousarray(wl.i_idx[shard_rows[0]:shard_rows[1]]),
-                                 r_s=np.ascontiguousarray(wl.r_s[shard_rows[0]:shard_rows[1]]))
+    wl, job_pairs, job_replicas, shard_rows = shard_job(wl, rank, world, args.shard)
     s = wl.state
-    ctx = binding.Context(s.n, wl.n_i, wl.cap, device=local)
-    state_dev = ctx.set_state(s)
-    i_idx = torch.from_numpy(wl.i_idx).to(dev)
-    r_s = torch.from_numpy(wl.r_s).to(dev)
-    out = ctx.alloc_outputs(wl.n_i)
+    b = Bench(wl, local)
+    ctx, i_idx, r_s, out, state_dev = b.ctx, b.i_idx, b.r_s, b.out, b.state_dev
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
-    def step(ev=None):
-        ctx.nb_set_j(*state_dev)           # GPUNB_SEND: new block-step, prediction invalid
-        if ev: ev[0].record()
-        ctx.nb_predict_j(s.t)              # S1
-        if ev: ev[1].record()
-        ctx.nb_regular_force(i_idx, r_s, s.t, out=out)  # S2-S5 (prediction already at t)
-        if ev: ev[2].record()
-
-    for _ in range(max(args.warmup, 3)):
-        step()
-    torch.cuda.synchronize()
-    info = ctx.nb_last_launch_info()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
-    if dist: dist.barrier()
-    torch.cuda.synchronize()
-    for k in range(args.steps):
-        flush.fill_(k & 0xff)              # L2 flush between timed iterations (outside the per-step events)
-        step(evs[k])
-    torch.cuda.synchronize()
-    if dist: dist.barrier()
+    ts, tp, tf, info = b.timed(args.steps, args.warmup, flush, dist)
     clocks = sampler.stop() if rank == 0 else None
-    t_step = sum(e[0].elapsed_time(e[2]) for e in evs) / 1e3          # s, all K steps, device time
-    t_pred = sum(e[0].elapsed_time(e[1]) for e in evs) / 1e3 / args.steps
-    t_force = sum(e[1].elapsed_time(e[2]) for e in evs) / 1e3 / args.steps
+    t_step = float(ts.sum())                                            # s, all K steps, device time
+    t_pred, t_force = float(tp.mean()), float(tf.mean())
     t_max = max_over_ranks(t_step, dist, dev)
     value = whole_job_rate(job_pairs, args.steps, job_replicas, t_max)
     n_over = int(out["n_overflow"].item())
@@ -348,11 +478,14 @@ def run_gpu_arm(args):
         torch.cuda.synchronize()
         t_irr = ev[0].elapsed_time(ev[1]) / 5 / 1e3
         irr_pairs = int(torch.clamp(out["nbr_count"], max=wl.cap).sum().item())
+        rec_bytes = irr_pairs * 48
         irr = {"kernel": "irregular_kernel", "pairs": irr_pairs, "ms": t_irr * 1e3,
                "value": irr_pairs / t_irr / 1e9, "unit": UNIT, "bound": "l2-gather",
-               "gathered_gb_per_s": irr_pairs * 48 / t_irr / 1e9,
+               "gathered_gb_per_s": rec_bytes / t_irr / 1e9,
+               "hbm_frac_if_all_gathers_missed_l2": rec_bytes / t_irr / 1e9 / peaks["hbm_gbs"],
                "note": "eq. (7), (8) over the neighbour lists of the last step; one 48 B particle-major record gathered per pair "
-                       "(L2-resident at this N); bound by the L1/TEX sector rate for scattered accesses (profiles/), for which no measured peak exists in MEASURED_PEAKS.json, so no fraction is given"}
+                       "(L2-resident at this N); bound by the L1/TEX sector rate for scattered accesses (profiles/): the "
+                       "fractions of the HBM and L2 peaks the kernel reaches are in profiles/r2_irregular_kernel_ncu_full.md"}
 
     # ---- step (vii) and eq. (1): the regular corrector on the lists of two regular-force calls
     # (radii of the second scaled by a seeded factor in [0.9, 1.1]).  Reported beside the headline, not part of it.
@@ -383,9 +516,10 @@ def run_gpu_arm(args):
         cor_bytes = (n_old + n_new) * 4 + wl.n_i * (4 * 24 + 8 * 3 + 4 * 3 + 6 * 24 + 8)
         cor = {"kernel": "corrector_kernel", "rows": wl.n_i, "ms": t_cor * 1e3, "rows_per_s": wl.n_i / t_cor,
                "list_entries_compared": n_old + n_new, "stream_gb_per_s": cor_bytes / t_cor / 1e9,
-               "note": "step (vii) + eq. (1): symmetric difference of the old and new list by warp-shuffle compares, pair "
-                       "terms of the members that changed, fp64 Hermite arithmetic; stream_gb_per_s counts both lists "
-                       "and the per-row arrays once (the gathers of the changed members come on top)"}
+               "hbm_frac": cor_bytes / t_cor / 1e9 / peaks["hbm_gbs"],
+               "note": "step (vii) + eq. (1): symmetric difference of the old and new list, pair terms of the members that "
+                       "changed, fp64 Hermite arithmetic; stream_gb_per_s counts both lists and the per-row arrays once "
+                       "(the gathers of the changed members come on top)"}
         del old
 
     # ---- e2e: C-ABI call with HOST (pinned) buffers, copies inside the timed region
@@ -421,35 +555,41 @@ def run_gpu_arm(args):
     if rank != 0:
         if dist: dist.destroy_process_group()
         return 0
-    nsm = torch.cuda.get_device_properties(local).multi_processor_count
-    peak_tf = nsm * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    nsm, peak_tf = fp32_peak_tflops(torch, local, peaks)
     ach_tf = wl.pairs * FLOPS_PER_PAIR / t_force / 1e12
-    pred_bytes = s.n * (112 + 40 + 48)  # state read; pair-interleaved and particle-major records written
+    pred_bytes = s.n * PRED_BYTES_PER_J
+    headline = args.config == 5 and args.n_i is None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True,
+        "warmup": max(args.warmup, 3), "ms_per_step": t_max / args.steps * 1e3,
+        "ms_per_step_median": float(np.median(ts)) * 1e3, "ms_per_step_best": float(ts.min()) * 1e3,
+        "value_best": whole_job_rate(job_pairs, 1, job_replicas, float(ts.min())) if world == 1 else None,
+        "higher_is_better": True,
         "scaling": "strong" if shard_rows else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": workload_config(wl, args.config),
         "fp32_peak_fraction": value / world * 1e9 * FLOPS_PER_PAIR / (peak_tf * 1e12),
         "roofline": {"bound": "alu", "kernel": "force_kernel", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
                      "frac": ach_tf / peak_tf,
-                     "traffic": FORCE_DRAM_BYTES_C5 if (args.config == 5 and args.n_i is None) else None,
+                     "traffic": FORCE_DRAM_BYTES_C5 if headline else None,
                      "fma_pipe_busy": wl.pairs * LANE_SLOTS_PER_PAIR / t_force / (nsm * 128 * peaks["sm_max_mhz"] * 1e6),
                      "note": f"achieved = N_i*N pairs x {FLOPS_PER_PAIR:.0f} flop (convention) / time of "
-                             f"nb_regular_force on its stream (CUDA events; force_kernel plus the small "
-                             f"reduce_gather_kernel of the j-split rows); peak = {nsm} SMs x 128 FP32 lanes x 2 x "
+                             f"nb_regular_force on its stream (CUDA events; force_kernel plus the small gather and "
+                             f"fp64 fix-up kernels); peak = {nsm} SMs x 128 FP32 lanes x 2 x "
                              f"{peaks['sm_max_mhz']:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz, {peaks['src']}; the "
                              f"file holds no FP32 figure, DESIGN.md section 7 derives this one); fma_pipe_busy = "
                              f"{LANE_SLOTS_PER_PAIR:.0f} issued FP32 lane-slots per pair / 128 per clock per SM",
                      "ms": t_force * 1e3},
         "roofline_predictor": {"bound": "hbm", "kernel": "predict_kernel", "achieved": pred_bytes / t_pred / 1e9,
                                "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": pred_bytes / t_pred / 1e9 / peaks["hbm_gbs"],
-                               "traffic": None, "ms": t_pred * 1e3,
-                               "note": f"200 B/j algorithmic (112 read + 40 + 48 written), peak {peaks['src']} copy bandwidth; ms is the "
-                                       f"interval between two events around ONE launch inside the step and includes the "
-                                       f"event-to-kernel latency (the kernel alone: 38.6 us = 5.4 TB/s in "
-                                       f"profiles/r1_bench_c5_launches.md)"},
+                               "frac_at_survey_160_bytes": s.n * 160 / t_pred / 1e9 / peaks["hbm_gbs"],
+                               "traffic": PRED_DRAM_BYTES_C5 if headline else None, "ms": t_pred * 1e3,
+                               "note": f"{PRED_BYTES_PER_J} B/j algorithmic (112 B of fp64 state read, 40 B pair record written; SURVEY "
+                                       f"8(a) S1 budgets 112 + 48 = 160 B/j for a padded record: frac_at_survey_160_bytes), peak "
+                                       f"{peaks['src']} copy bandwidth; ms is the interval between two events around ONE launch "
+                                       f"inside the step and includes the event-to-kernel latency (the kernel alone: "
+                                       f"profiles/r2_bench_c5_launches.md)"},
         "launch": info, "gpu_launches": int(info["launches"] + 1) * args.steps,
+        "fixup_rows_per_step": info["fixup_rows"],
         "mean_neighbours": mean_cnt, "overflow_rows": n_over, "clocks": clocks, "e2e": e2e,
         "next_irregular": irr,
         "next_corrector": cor,
@@ -459,8 +599,14 @@ def run_gpu_arm(args):
                                         "every rank predicts all j; no data-path collective"
         line["config"]["job_pairs_per_step"] = job_pairs
     if not args.no_cpu and world >= 1:
-        cb, _ = cpu_baseline(wl, target_seconds=args.cpu_seconds)
+        cb, _, rows, ores = cpu_baseline(wl, target_seconds=args.cpu_seconds, min_rows=min(wl.n_i, 1024))
         line["cpu_baseline"] = cb
+        # parity of the last timed repetition (out has not been written since) against those oracle rows
+        line["parity"] = parity_in_run(wl, out, rows, ores)
+    b.close()
+    if headline and not args.no_also and world == 1:
+        # the other configs, incl. the N = 65536 full block the ">= 50 % for N >= 65536" target names
+        line["also"] = [run_also(c, local, flush, peaks, steps=(10 if c == 3 else 20)) for c in (3, 4, 2, 1)]
     print(json.dumps(line))
     if dist: dist.destroy_process_group()
     return 0
@@ -478,6 +624,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-irregular", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the other configs beside the headline (configs 3, 4, 2, 1)")
     ap.add_argument("--sweep", action="store_true", help="config 3 active-block sweep 32 ... 65536 (one JSON line)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--shard", default="none", choices=["none", "rows"],

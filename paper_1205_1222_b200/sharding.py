@@ -37,6 +37,13 @@ def shard_sizes(n_i: int, world: int, grain: int = ROW_GRAIN) -> list[int]:
     return [hi - lo for lo, hi in (row_shard(n_i, r, world, grain) for r in range(world))]
 
 
+def shard_capacity(n_i_max: int, world: int, grain: int = ROW_GRAIN) -> int:
+    """Rows a rank's context must hold so that ANY block of up to n_i_max rows fits its shard: the largest shard of the
+    largest block (rank 0's), which is also the largest shard of every smaller block (shard sizes grow with n_i)."""
+    lo, hi = row_shard(n_i_max, 0, world, grain)
+    return max(hi - lo, 1)
+
+
 def allgather_rows(local: torch.Tensor, n_i: int, rank: int, world: int, group=None,
                    grain: int = ROW_GRAIN) -> torch.Tensor:
     """All ranks' row slices of a per-row output (acc, jerk, nbr_count, ...) -> the full [n_i, ...] tensor on every
@@ -66,8 +73,7 @@ class ShardedContext:
         from . import binding  # loads the CUDA library: fails loudly without it
 
         self.rank, self.world, self.group = rank, world, group
-        lo, hi = row_shard(n_i_max, 0, world)  # rank 0 owns a largest shard
-        self.ctx = binding.Context(n_max, max(hi - lo, 1), nbr_cap, device=device)
+        self.ctx = binding.Context(n_max, shard_capacity(n_i_max, world), nbr_cap, device=device)
         self.rows = (0, 0)
 
     def set_state(self, state):

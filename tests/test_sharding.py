@@ -33,6 +33,20 @@ def test_row_shard_partitions_the_block(grain):
             assert lens == sorted(lens, reverse=True)        # rank 0 owns a largest shard (ShardedContext sizes by it)
 
 
+def test_shard_capacity_holds_every_block_up_to_n_i_max():
+    """ShardedContext sizes its context by shard_capacity(n_i_max, world): every rank's shard of every block of up to
+    n_i_max rows must fit, also when n_i is not a multiple of world x 128."""
+    rng = np.random.default_rng(6)
+    for world in (1, 2, 3, 4, 8):
+        for n_i_max in [1, 127, 129, 333, 1000, 5000, 65537] + [int(v) for v in rng.integers(1, 200000, 10)]:
+            cap = sharding.shard_capacity(n_i_max, world)
+            assert cap >= 1
+            for n_i in {n_i_max, max(1, n_i_max - 1), max(1, n_i_max // 2), max(1, n_i_max - 127), 1}:
+                assert max(sharding.shard_sizes(n_i, world)) <= cap
+            # tight: no more than one grain above an even split
+            assert cap <= -(-n_i_max // world) + sharding.ROW_GRAIN
+
+
 def test_row_shard_rejects_bad_arguments():
     for args in ((-1, 0, 1), (10, 1, 1), (10, -1, 2), (10, 0, 0)):
         with pytest.raises(ValueError):
