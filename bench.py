@@ -528,28 +528,31 @@ def run_gpu_arm(args):
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
         h_in = [pin(a) for a in (s.x0, s.v0, s.a0, s.j0, s.m, s.t0)]
         h_idx, h_rs = pin(wl.i_idx), pin(wl.r_s)
+        # the lists come back in CSR form (nb_regular_force_host_csr): the stored entries packed back to back
+        stored = int(torch.clamp(out["nbr_count"], max=wl.cap).sum().item())
         h_out = dict(acc=torch.empty((wl.n_i, 3), dtype=torch.float64).pin_memory(),
                      jerk=torch.empty((wl.n_i, 3), dtype=torch.float64).pin_memory(),
                      nbr_count=torch.empty(wl.n_i, dtype=torch.int32).pin_memory(),
-                     nbr_list=torch.empty((wl.n_i, wl.cap), dtype=torch.int32).pin_memory(),
+                     nbr_offset=torch.empty(wl.n_i + 1, dtype=torch.int64).pin_memory(),
+                     nbr_packed=torch.empty(stored + stored // 16 + 1024, dtype=torch.int32).pin_memory(),
                      n_overflow=torch.zeros(1, dtype=torch.int32).pin_memory())
         h2d = sum(t.numel() * t.element_size() for t in h_in + [h_idx, h_rs])
-        # device -> host: acc, jerk, counts, n_overflow in full; of the (n_i x cap) list array only the columns up to
-        # the longest stored list, rounded up to 32 (what nb_regular_force_host copies)
-        width = min(wl.cap, -(-int(torch.clamp(out["nbr_count"], max=wl.cap).max().item()) // 32) * 32)
-        d2h = wl.n_i * (24 + 24 + 4 + 4 * width) + 4
+        # device -> host: acc, jerk, counts, row offsets, n_overflow in full, and the stored list entries
+        d2h = wl.n_i * (24 + 24 + 4 + 8) + 8 + 4 + 4 * stored
         ksteps = max(1, min(args.steps, 3))
-        ctx.nb_regular_force_host(*h_in, h_idx, h_rs, s.t, h_out)  # warm-up (allocates the mirrors)
+        ctx.nb_regular_force_host_csr(*h_in, h_idx, h_rs, s.t, h_out)  # warm-up (allocates the mirrors)
         if dist: dist.barrier()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         for _ in range(ksteps):
-            ctx.nb_regular_force_host(*h_in, h_idx, h_rs, s.t, h_out)  # synchronises internally
+            ctx.nb_regular_force_host_csr(*h_in, h_idx, h_rs, s.t, h_out)  # synchronises internally
         te = time.perf_counter() - t0
         te_max = max_over_ranks(te, dist, dev)
         e2e = {"value": whole_job_rate(job_pairs, ksteps, job_replicas, te_max), "unit": UNIT,
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "steps": ksteps,
-               "ms_per_step": te_max / ksteps * 1e3, "api": "nb_regular_force_host (pinned host buffers)"}
+               "ms_per_step": te_max / ksteps * 1e3,
+               "api": "nb_regular_force_host_csr (pinned host buffers; neighbour lists returned in CSR form)",
+               "lists_match_device_run": bool(int(h_out["nbr_offset"][-1]) == stored)}
         ctx.nb_set_j(*state_dev)
 
     if rank != 0:

@@ -210,6 +210,20 @@ int nb_regular_force_host(nb_ctx* ctx, int64_t n, const double* x0, const double
                           const double* r_s, double t, double* acc, double* jerk, int32_t* nbr_count,
                           int32_t* nbr_list, int32_t* n_overflow);
 
+/* The same call returning the neighbour lists in CSR form, which is what a host integrator stores anyway and a
+ * fraction of the bytes of the dense [n_i][nbr_cap] rectangle (config 5: ~100 of 512 columns used): the stored entries
+ * min(count, nbr_cap) of all rows back to back, packed on the device (exclusive scan + one warp per row) before they
+ * travel.
+ *   nbr_offset:  host int64[n_i + 1]   row q's entries are nbr_packed[nbr_offset[q] .. nbr_offset[q + 1]), ascending j
+ *   nbr_packed:  host int32[packed_capacity]
+ * If the entries do not fit packed_capacity the call returns NB_E_NOMEM after filling acc, jerk, nbr_count, n_overflow
+ * and nbr_offset (nbr_offset[n_i] is the capacity to come back with); nbr_packed then holds the leading row chunks
+ * that did fit.  Everything else as nb_regular_force_host. */
+int nb_regular_force_host_csr(nb_ctx* ctx, int64_t n, const double* x0, const double* v0, const double* a0,
+                              const double* j0, const double* m, const double* t0, int32_t n_i, const int32_t* i_idx,
+                              const double* r_s, double t, double* acc, double* jerk, int32_t* nbr_count,
+                              int64_t* nbr_offset, int32_t* nbr_packed, int64_t packed_capacity, int32_t* n_overflow);
+
 /* The fp64 fix-up pass (footnote 2: "options using the 'two-float' method for the coordinates and the
  * accumulator").  The pair arithmetic of nb_regular_force[_ex] is fp32, so a row's absolute error is
  * ~ eps sqrt(sum_j |term_j|^2) whatever its sum comes to; rows whose terms cancel would miss the per-particle bound

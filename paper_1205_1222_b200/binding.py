@@ -53,6 +53,7 @@ def load(build_if_missing: bool = True):
     lib.nb_irregular_force_act.argtypes = [vp, i32, vp, vp, vp, i32, dbl, vp, vp, vp]
     lib.nb_regular_correct.argtypes = [vp, i32, ctypes.POINTER(CorrectorIO), dbl, vp]
     lib.nb_regular_force_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp]
+    lib.nb_regular_force_host_csr.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp, i64, vp]
     lib.nb_set_option.argtypes = [vp, ctypes.c_char_p, i64]
     lib.nb_get_error_scale.argtypes = [vp, i32, vp, vp]
     lib.nb_fixup_stats.argtypes = [vp, ctypes.POINTER(i64), vp]
@@ -245,6 +246,20 @@ class Context:
             _host(m, f64, "m"), _host(t0, f64, "t0"), n_i, _host(i_idx, torch.int32, "i_idx"),
             _host(r_s, f64, "r_s"), float(t), _host(out["acc"], f64, "acc"), _host(out["jerk"], f64, "jerk"),
             _host(out["nbr_count"], torch.int32, "nbr_count"), _host(out["nbr_list"], torch.int32, "nbr_list"),
+            _host(out["n_overflow"], torch.int32, "n_overflow")))
+        self.n = n
+        return out
+
+    def nb_regular_force_host_csr(self, x0, v0, a0, j0, m, t0, i_idx, r_s, t: float, out):
+        """Lists in CSR form: out["nbr_offset"] int64 [n_i + 1], out["nbr_packed"] int32 [capacity] (CPU tensors)."""
+        f64 = torch.float64
+        n, n_i = int(x0.shape[0]), int(i_idx.shape[0])
+        _check(self.lib.nb_regular_force_host_csr(
+            self._h, n, _host(x0, f64, "x0"), _host(v0, f64, "v0"), _host(a0, f64, "a0"), _host(j0, f64, "j0"),
+            _host(m, f64, "m"), _host(t0, f64, "t0"), n_i, _host(i_idx, torch.int32, "i_idx"),
+            _host(r_s, f64, "r_s"), float(t), _host(out["acc"], f64, "acc"), _host(out["jerk"], f64, "jerk"),
+            _host(out["nbr_count"], torch.int32, "nbr_count"), _host(out["nbr_offset"], torch.int64, "nbr_offset"),
+            _host(out["nbr_packed"], torch.int32, "nbr_packed"), int(out["nbr_packed"].numel()),
             _host(out["n_overflow"], torch.int32, "n_overflow")))
         self.n = n
         return out

@@ -242,4 +242,24 @@ __global__ void __launch_bounds__(256) list_width_kernel(const int32_t* nbr_coun
     if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
 }
 
+// Host entry point, CSR form: stored entries min(count, cap) of a row (the scan's input), and the packing of the rows'
+// stored entries back to back at their offsets (one warp per row, coalesced).
+struct StoredLen {
+    const int32_t* cnt;
+    int32_t cap;
+    __host__ __device__ int64_t operator()(int64_t q) const { return (int64_t)min(cnt[q], cap); }
+};
+
+__global__ void __launch_bounds__(kGatherWarps * 32) pack_lists_kernel(const int32_t* nbr_count, const int32_t* nbr_list,
+                                                                      int32_t n_rows, int32_t cap, const int64_t* offset,
+                                                                      int32_t* packed) {
+    const int lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * kGatherWarps + (threadIdx.x >> 5);
+    if (row >= n_rows) return;
+    const int32_t len = min(nbr_count[row], cap);
+    const int32_t* src = nbr_list + (size_t)row * cap;
+    int32_t* dst = packed + offset[row];
+    for (int32_t e = lane; e < len; e += 32) dst[e] = src[e];
+}
+
 }  // namespace nbreg

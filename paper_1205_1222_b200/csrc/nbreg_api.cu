@@ -9,6 +9,9 @@
 #include <utility>
 
 #include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
+#include <thrust/iterator/counting_iterator.h>
+#include <thrust/iterator/transform_iterator.h>
 #include <new>
 
 #include "force.cuh"
@@ -182,6 +185,7 @@ struct nb_ctx {
     int32_t* hovf = nullptr;                          // pinned: overflow count, then longest list, of each chunk
     unsigned char* hbuf = nullptr;
     size_t hbuf_bytes = 0;
+    unsigned char* hcsr = nullptr;                    // CSR host path: packed lists, row offsets, scan scratch
 };
 
 namespace {
@@ -524,6 +528,7 @@ int nb_destroy(nb_ctx* c) {
         if (c->hdone[k]) cudaEventDestroy(c->hdone[k]);
     if (c->hovf) cudaFreeHost(c->hovf);
     if (c->hbuf) cudaFree(c->hbuf);
+    if (c->hcsr) cudaFree(c->hcsr);
     if (c->ws_owned && c->ws) cudaFree(c->ws);
     delete c;
     return NB_OK;
@@ -836,15 +841,31 @@ int nb_regular_correct(nb_ctx* c, int32_t n_i, const nb_corrector_io* io, double
 static int regular_force_host_impl(nb_ctx* c, int64_t n, const double* x0, const double* v0, const double* a0,
                                    const double* j0, const double* m, const double* t0, int32_t n_i,
                                    const int32_t* i_idx, const double* r_s, double t, double* acc, double* jerk,
-                                   int32_t* nbr_count, int32_t* nbr_list, int32_t* n_overflow);
+                                   int32_t* nbr_count, int32_t* nbr_list, int64_t* nbr_offset, int32_t* nbr_packed,
+                                   int64_t packed_capacity, int32_t* n_overflow);
 
 int nb_regular_force_host(nb_ctx* c, int64_t n, const double* x0, const double* v0, const double* a0,
                           const double* j0, const double* m, const double* t0, int32_t n_i, const int32_t* i_idx,
                           const double* r_s, double t, double* acc, double* jerk, int32_t* nbr_count,
                           int32_t* nbr_list, int32_t* n_overflow) {
+    if (n_i > 0 && !nbr_list) return NB_E_INVAL;
     const int rc = regular_force_host_impl(c, n, x0, v0, a0, j0, m, t0, n_i, i_idx, r_s, t, acc, jerk, nbr_count,
-                                           nbr_list, n_overflow);
+                                           nbr_list, nullptr, nullptr, 0, n_overflow);
     if (rc != NB_OK && c) {  // leave nothing of this call in flight: the caller may free or reuse its host buffers
+        if (c->hstream) cudaStreamSynchronize(c->hstream);
+        if (c->hcopy) cudaStreamSynchronize(c->hcopy);
+    }
+    return rc;
+}
+
+int nb_regular_force_host_csr(nb_ctx* c, int64_t n, const double* x0, const double* v0, const double* a0,
+                              const double* j0, const double* m, const double* t0, int32_t n_i, const int32_t* i_idx,
+                              const double* r_s, double t, double* acc, double* jerk, int32_t* nbr_count,
+                              int64_t* nbr_offset, int32_t* nbr_packed, int64_t packed_capacity, int32_t* n_overflow) {
+    if (!nbr_offset || packed_capacity < 0 || (packed_capacity > 0 && !nbr_packed)) return NB_E_INVAL;
+    const int rc = regular_force_host_impl(c, n, x0, v0, a0, j0, m, t0, n_i, i_idx, r_s, t, acc, jerk, nbr_count,
+                                           nullptr, nbr_offset, nbr_packed, packed_capacity, n_overflow);
+    if (rc != NB_OK && c) {
         if (c->hstream) cudaStreamSynchronize(c->hstream);
         if (c->hcopy) cudaStreamSynchronize(c->hcopy);
     }
@@ -854,16 +875,18 @@ int nb_regular_force_host(nb_ctx* c, int64_t n, const double* x0, const double* 
 static int regular_force_host_impl(nb_ctx* c, int64_t n, const double* x0, const double* v0, const double* a0,
                                    const double* j0, const double* m, const double* t0, int32_t n_i,
                                    const int32_t* i_idx, const double* r_s, double t, double* acc, double* jerk,
-                                   int32_t* nbr_count, int32_t* nbr_list, int32_t* n_overflow) {
+                                   int32_t* nbr_count, int32_t* nbr_list, int64_t* nbr_offset, int32_t* nbr_packed,
+                                   int64_t packed_capacity, int32_t* n_overflow) {
+    const bool csr = nbr_offset != nullptr;
     if (!c || !x0 || !v0 || !a0 || !j0 || !m || !t0 || !n_overflow) return NB_E_INVAL;
     if (n < 1 || n > c->n_max || n_i < 0 || n_i > c->n_i_max) return NB_E_INVAL;
-    if (n_i > 0 && (!i_idx || !r_s || !acc || !jerk || !nbr_count || !nbr_list)) return NB_E_INVAL;
+    if (n_i > 0 && (!i_idx || !r_s || !acc || !jerk || !nbr_count)) return NB_E_INVAL;
     NB_CUDA(cudaSetDevice(c->device));
     if (!c->hstream) NB_CUDA(cudaStreamCreateWithFlags(&c->hstream, cudaStreamNonBlocking));
     if (!c->hcopy) NB_CUDA(cudaStreamCreateWithFlags(&c->hcopy, cudaStreamNonBlocking));
     for (int k = 0; k < kHostChunks; ++k)
         if (!c->hdone[k]) NB_CUDA(cudaEventCreateWithFlags(&c->hdone[k], cudaEventDisableTiming));
-    if (!c->hovf) NB_CUDA(cudaMallocHost(&c->hovf, 2 * kHostChunks * sizeof(int32_t)));
+    if (!c->hovf) NB_CUDA(cudaMallocHost(&c->hovf, 2 * kHostChunks * sizeof(int32_t) + kHostChunks * sizeof(int64_t)));
     // device mirrors, carved from one allocation sized for n_max / n_i_max / cap
     const size_t nmax = (size_t)c->n_max, imax = (size_t)c->n_i_max;
     size_t off = 0;
@@ -880,6 +903,28 @@ static int regular_force_host_impl(nb_ctx* c, int64_t n, const double* x0, const
         }
         c->hbuf_bytes = off;
     }
+    // CSR mode: the stored entries of every row packed back to back (first use allocates; worst case n_i_max x cap),
+    // row offsets (local to a row chunk), and the scan's scratch
+    size_t scan_temp = 0;
+    if (csr) {
+        StoredLen f{nullptr, c->cap};
+        auto it = thrust::make_transform_iterator(thrust::counting_iterator<int64_t>(0), f);
+        cub::DeviceScan::ExclusiveSum(nullptr, scan_temp, it, (int64_t*)nullptr, (int)std::max<int64_t>(c->n_i_max, 1));
+        scan_temp = (size_t)round_up((int64_t)scan_temp, 256) + 256;
+        if (!c->hcsr) {
+            const size_t bytes = (size_t)round_up((int64_t)(imax * (size_t)c->cap * 4), 256) +
+                                 (size_t)round_up((int64_t)((imax + 1) * 8), 256) + scan_temp + 256;
+            if (cudaMalloc(&c->hcsr, bytes) != cudaSuccess) {
+                cudaGetLastError();
+                return NB_E_NOMEM;
+            }
+        }
+    }
+    int32_t* d_packed = reinterpret_cast<int32_t*>(c->hcsr);
+    int64_t* d_off = csr ? reinterpret_cast<int64_t*>(c->hcsr + (size_t)round_up((int64_t)(imax * (size_t)c->cap * 4), 256))
+                         : nullptr;
+    unsigned char* d_scan = csr ? reinterpret_cast<unsigned char*>(d_off) + (size_t)round_up((int64_t)((imax + 1) * 8), 256)
+                                : nullptr;
     unsigned char* b = c->hbuf;
     cudaStream_t st = c->hstream, cs = c->hcopy;
     const size_t nn = (size_t)n, ni = (size_t)n_i, cap = (size_t)c->cap;
@@ -897,17 +942,22 @@ static int regular_force_host_impl(nb_ctx* c, int64_t n, const double* x0, const
                       (const double*)(b + o_j0), (const double*)(b + o_m), (const double*)(b + o_t0));
     if (rc != NB_OK) return rc;
     // row chunks: compute chunk k on the compute stream, copy its rows back on the copy stream meanwhile
-    // ... when that pays: a row costs ~N ns of compute per 1000 j and (4 cap + 52) B of copy at ~50 GB/s; splitting a
-    // block costs a few per cent of kernel efficiency, so it is done only if the copy is >= 10 % of the compute
-    const bool overlap_pays = (double)(4 * (int64_t)c->cap + 52) / 50.0 >= 0.1 * (double)n / 1000.0;
+    // ... when that pays: a row costs ~N ns of compute per 1000 j and (4 cap + 52) B of copy at ~50 GB/s (dense lists;
+    // ~4 x 100 + 60 B in CSR form); splitting a block costs a few per cent of kernel efficiency, so it is done only if
+    // the copy is >= 10 % of the compute
+    const double row_bytes = csr ? 460.0 : (double)(4 * (int64_t)c->cap + 52);
+    const bool overlap_pays = row_bytes / 50.0 >= 0.1 * (double)n / 1000.0;
     int64_t rows_per_chunk = std::max<int64_t>(kHostChunkMinRows, (n_i + kHostChunks - 1) / kHostChunks);
     rows_per_chunk = round_up(rows_per_chunk, 1024);
     if (!overlap_pays) rows_per_chunk = round_up(std::max<int64_t>(n_i, 1), 1024);
     const int n_chunks = n_i > 0 ? (int)((n_i + rows_per_chunk - 1) / rows_per_chunk) : 1;
-    // first everything that computes, then, chunk by chunk as they finish, the copies: only the columns of nbr_list
-    // that hold entries travel (the longest stored list of the chunk, rounded up to 32 columns)
+    // first everything that computes, then, chunk by chunk as they finish, the copies.  Dense mode: only the columns of
+    // nbr_list that hold entries travel (the longest stored list of the chunk, rounded up to 32).  CSR mode: the stored
+    // entries are packed on the device (exclusive scan of min(count, cap) + one warp per row) and travel back to back.
     int32_t* d_ovf = (int32_t*)(b + o_ovf);          // [kHostChunks] overflow counts
     int32_t* d_wid = d_ovf + kHostChunks;            // [kHostChunks] longest stored lists
+    int64_t* d_tot = (int64_t*)(d_wid + kHostChunks);  // [kHostChunks] stored entries of each chunk (CSR)
+    int64_t* h_tot = (int64_t*)(c->hovf + 2 * kHostChunks);
     NB_CUDA(cudaMemsetAsync(d_wid, 0, kHostChunks * sizeof(int32_t), st));
     for (int k = 0; k < n_chunks; ++k) {
         const size_t r0 = (size_t)k * (size_t)rows_per_chunk;
@@ -916,35 +966,74 @@ static int regular_force_host_impl(nb_ctx* c, int64_t n, const double* x0, const
                               (double*)(b + o_acc) + 3 * r0, (double*)(b + o_jrk) + 3 * r0, (int32_t*)(b + o_cnt) + r0,
                               (int32_t*)(b + o_lst) + r0 * cap, d_ovf + k, st);
         if (rc != NB_OK) return rc;
-        if (nr > 0) {
+        if (nr > 0 && !csr) {
             const unsigned blocks = (unsigned)std::min<size_t>((nr + 255) / 256, 1024);
             list_width_kernel<<<blocks, 256, 0, st>>>((const int32_t*)(b + o_cnt) + r0, (int32_t)nr, c->cap, d_wid + k);
             NB_CUDA(cudaGetLastError());
+        }
+        if (csr) {  // offsets of the chunk's rows (local: the chunk's first row starts at 0), its total, the packed entries
+            StoredLen f{(const int32_t*)(b + o_cnt) + r0, c->cap};
+            auto it = thrust::make_transform_iterator(thrust::counting_iterator<int64_t>(0), f);
+            size_t temp = scan_temp;
+            NB_CUDA(cub::DeviceScan::ExclusiveSum(d_scan, temp, it, d_off + r0, (int)nr + 1, st));  // [nr] = the total
+            NB_CUDA(cudaMemcpyAsync(d_tot + k, d_off + r0 + nr, sizeof(int64_t), cudaMemcpyDeviceToDevice, st));
+            if (nr > 0) {
+                const unsigned blocks = (unsigned)((nr + kGatherWarps - 1) / kGatherWarps);
+                pack_lists_kernel<<<blocks, kGatherWarps * 32, 0, st>>>((const int32_t*)(b + o_cnt) + r0,
+                                                                       (const int32_t*)(b + o_lst) + r0 * cap, (int32_t)nr,
+                                                                       c->cap, d_off + r0, d_packed + r0 * cap);
+                NB_CUDA(cudaGetLastError());
+            }
+            NB_CUDA(cudaMemcpyAsync(h_tot + k, d_tot + k, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
         }
         NB_CUDA(cudaMemcpyAsync(c->hovf + k, d_ovf + k, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
         NB_CUDA(cudaMemcpyAsync(c->hovf + kHostChunks + k, d_wid + k, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
         NB_CUDA(cudaEventRecord(c->hdone[k], st));
     }
+    int64_t base = 0;      // CSR: entries of the chunks before this one
+    int64_t bases[kHostChunks + 1] = {0};
+    bool fits = true;
     for (int k = 0; k < n_chunks; ++k) {
         const size_t r0 = (size_t)k * (size_t)rows_per_chunk;
         const size_t nr = n_i > 0 ? std::min<size_t>((size_t)rows_per_chunk, ni - r0) : 0;
-        NB_CUDA(cudaEventSynchronize(c->hdone[k]));  // chunk k is final on the device, its list width is known
+        NB_CUDA(cudaEventSynchronize(c->hdone[k]));  // chunk k is final on the device, its list width / total is known
+        bases[k] = base;
         if (nr == 0) continue;
         NB_CUDA(cudaMemcpyAsync(acc + 3 * r0, (double*)(b + o_acc) + 3 * r0, nr * 24, cudaMemcpyDeviceToHost, cs));
         NB_CUDA(cudaMemcpyAsync(jerk + 3 * r0, (double*)(b + o_jrk) + 3 * r0, nr * 24, cudaMemcpyDeviceToHost, cs));
         NB_CUDA(cudaMemcpyAsync(nbr_count + r0, (int32_t*)(b + o_cnt) + r0, nr * 4, cudaMemcpyDeviceToHost, cs));
-        const size_t width = std::min<size_t>(cap, (size_t)round_up(c->hovf[kHostChunks + k], 32));
-        if (width > 0)
-            NB_CUDA(cudaMemcpy2DAsync(nbr_list + r0 * cap, cap * 4, (int32_t*)(b + o_lst) + r0 * cap, cap * 4, width * 4,
-                                      nr, cudaMemcpyDeviceToHost, cs));
+        if (csr) {
+            const int64_t tot = h_tot[k];
+            NB_CUDA(cudaMemcpyAsync(nbr_offset + r0, d_off + r0, nr * 8, cudaMemcpyDeviceToHost, cs));
+            if (base + tot <= packed_capacity) {
+                if (tot > 0)
+                    NB_CUDA(cudaMemcpyAsync(nbr_packed + base, d_packed + r0 * cap, (size_t)tot * 4, cudaMemcpyDeviceToHost, cs));
+            } else {
+                fits = false;  // offsets and counts still arrive, so the caller knows the size to come back with
+            }
+            base += tot;
+        } else {
+            const size_t width = std::min<size_t>(cap, (size_t)round_up(c->hovf[kHostChunks + k], 32));
+            if (width > 0)
+                NB_CUDA(cudaMemcpy2DAsync(nbr_list + r0 * cap, cap * 4, (int32_t*)(b + o_lst) + r0 * cap, cap * 4, width * 4,
+                                          nr, cudaMemcpyDeviceToHost, cs));
+        }
     }
     NB_CUDA(cudaStreamSynchronize(st));
     NB_CUDA(cudaStreamSynchronize(cs));
+    if (csr) {  // chunk-local offsets -> global
+        for (int k = 1; k < n_chunks; ++k) {
+            const size_t r0 = (size_t)k * (size_t)rows_per_chunk;
+            const size_t nr = std::min<size_t>((size_t)rows_per_chunk, ni - r0);
+            for (size_t q = 0; q < nr; ++q) nbr_offset[r0 + q] += bases[k];
+        }
+        nbr_offset[ni] = base;
+    }
     int32_t total_overflow = 0;
     for (int k = 0; k < n_chunks; ++k) total_overflow += c->hovf[k];
     *n_overflow = total_overflow;
     // the registered pointers are the context's own mirrors; they stay valid, but a new host call overwrites them
-    return NB_OK;
+    return fits ? NB_OK : NB_E_NOMEM;
 }
 
 int nb_get_error_scale(nb_ctx* c, int32_t n_i, float* escale, void* stream) {

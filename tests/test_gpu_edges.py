@@ -300,6 +300,46 @@ def test_host_entry_point_in_row_chunks(oracle):
     ctx.close()
 
 
+@pytest.mark.parametrize("n,n_i", [(3001, 257), (2500, 40001), (900, 0)])
+def test_host_entry_point_csr_lists(oracle, n, n_i):
+    """nb_regular_force_host_csr: the same outputs with the lists packed back to back (CSR), in one chunk and in several
+    row chunks (40001 rows: three), overflowing rows cut at cap; too small a buffer is reported with the size needed."""
+    wl = _wl(oracle, n, max(n_i, 1), 20, 32)
+    if n_i == 0:
+        wl = inputs.Workload(wl.state, wl.i_idx[:0].copy(), wl.r_s[:0].copy(), wl.k, wl.cap)
+    wl.r_s[::1000] *= 3.0
+    s = wl.state
+    ctx = binding.Context(s.n, max(wl.n_i, 1), wl.cap)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_in = [pin(a) for a in (s.x0, s.v0, s.a0, s.j0, s.m, s.t0)] + [pin(wl.i_idx.astype(np.int32)), pin(wl.r_s)]
+    dense = dict(acc=torch.empty((wl.n_i, 3), dtype=torch.float64), jerk=torch.empty((wl.n_i, 3), dtype=torch.float64),
+                 nbr_count=torch.empty(wl.n_i, dtype=torch.int32),
+                 nbr_list=torch.full((wl.n_i, wl.cap), -7, dtype=torch.int32), n_overflow=torch.zeros(1, dtype=torch.int32))
+    ctx.nb_regular_force_host(*h_in, s.t, dense)
+    stored = np.minimum(dense["nbr_count"].numpy(), wl.cap).astype(np.int64)
+    total = int(stored.sum())
+    csr = dict(acc=torch.empty((wl.n_i, 3), dtype=torch.float64), jerk=torch.empty((wl.n_i, 3), dtype=torch.float64),
+               nbr_count=torch.empty(wl.n_i, dtype=torch.int32), nbr_offset=torch.full((wl.n_i + 1,), -1, dtype=torch.int64),
+               nbr_packed=torch.full((total + 5,), -7, dtype=torch.int32), n_overflow=torch.zeros(1, dtype=torch.int32))
+    ctx.nb_regular_force_host_csr(*h_in, s.t, csr)
+    for k in ("acc", "jerk", "nbr_count", "n_overflow"):
+        assert torch.equal(csr[k], dense[k]), k
+    off = csr["nbr_offset"].numpy()
+    assert np.array_equal(off, np.concatenate([[0], np.cumsum(stored)]))
+    packed = csr["nbr_packed"].numpy()
+    assert np.all(packed[total:] == -7)  # nothing written past the entries
+    ref = dense["nbr_list"].numpy()
+    for q in range(0, wl.n_i, max(1, wl.n_i // 3000)):
+        assert np.array_equal(packed[off[q]:off[q + 1]], ref[q, : stored[q]])
+    if wl.n_i > 0:  # a buffer that is too small: NB_E_NOMEM, and the offsets say what is needed
+        csr["nbr_packed"] = torch.empty(max(total // 2, 1), dtype=torch.int32)
+        csr["nbr_offset"].fill_(-1)
+        with pytest.raises(binding.NbregError):
+            ctx.nb_regular_force_host_csr(*h_in, s.t, csr)
+        assert int(csr["nbr_offset"][-1]) == total and torch.equal(csr["nbr_count"], dense["nbr_count"])
+    ctx.close()
+
+
 @pytest.mark.parametrize("n_i", [300, 4096, 4097, 8192, 9001])
 def test_row_ordering_paths(oracle, n_i):
     """Rows processed in Morton order of the predicted positions (one-CTA sorts of 512 x 8 and 1024 x 8 rows, device-wide

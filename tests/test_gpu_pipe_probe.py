@@ -1,0 +1,39 @@
+"""What the FP32 pipe of this GPU sustains for the packed f32x2 instructions force_kernel is made of (-m gpu).
+
+DESIGN.md section 5.2 argues that force_kernel (25 packed instructions per two pairs) sits close to what the pipe can
+deliver for its instruction mix, which is below the nominal 128 lanes per clock per SM.  That argument rests on this
+measurement: tests/probes/fp32x2_pipe_probe.cu, built here with nvcc for sm_100a and run on cuda:0.  The test keeps
+the claim honest: if a plain stream of three-operand FFMA2 ran at the nominal rate, the "practical ceiling" of the
+design notes would be wrong and the kernel would have more headroom than stated.
+The kept run: profiles/r2_fp32x2_pipe_probe.md."""
+import json
+import os
+import shutil
+import subprocess
+import tempfile
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def test_packed_fp32_pipe_rates():
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    src = os.path.join(HERE, "probes", "fp32x2_pipe_probe.cu")
+    with tempfile.TemporaryDirectory() as tmp:
+        exe = os.path.join(tmp, "fp32x2_pipe_probe")
+        subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-o", exe, src],
+                       check=True, capture_output=True)
+        out = subprocess.run([exe], check=True, capture_output=True, text=True).stdout
+    r = json.loads(out)
+    print("fp32x2 pipe probe:", r)
+    nominal = r["nominal_lanes_per_clk_per_sm"]
+    for k in ("ffma2_3reg", "ffma2_shared", "fadd2", "fmul2", "mix", "mix_mufu", "ffma_scalar"):
+        assert 0.3 * nominal < r[k] <= 1.02 * nominal, (k, r[k])
+    # the two-operand packed instructions run near the nominal rate ...
+    assert r["fadd2"] > 0.9 * nominal and r["fmul2"] > 0.9 * nominal
+    # ... the kernel's mix with its MUFU share cannot be faster than the plain mix
+    assert r["mix_mufu"] <= r["mix"] * 1.01
+    if os.path.isdir(os.path.join(os.path.dirname(HERE), "gpurun_out")):
+        json.dump(r, open(os.path.join(os.path.dirname(HERE), "gpurun_out", "pipe_probe.json"), "w"))
