@@ -99,12 +99,12 @@ _INFO_KEYS = ("rows_per_cta", "i_per_thread", "j_chunks", "ctas", "split_row_blo
 
 def nb_plan(n: int, n_i: int, num_sms: int = 148, ctas_per_sm=(3, 6, 12, 24, 1), i_block: int = 0,
             j_split: int = 0) -> dict:
-    """The launch planner alone (host only).  Same keys as nb_last_launch_info, with tiles_per_chunk in place
-    of launches."""
+    """The launch planner alone (host only).  Same keys as nb_last_launch_info, with chunk_j (particles per j-chunk)
+    in place of launches."""
     arr = (ctypes.c_int64 * 8)()
     occ = (ctypes.c_int32 * 5)(*[int(v) for v in ctas_per_sm])
     _check(load().nb_plan(int(n), int(n_i), int(num_sms), occ, int(i_block), int(j_split), arr))
-    keys = tuple("tiles_per_chunk" if k == "launches" else k for k in _INFO_KEYS)
+    keys = tuple("chunk_j" if k == "launches" else k for k in _INFO_KEYS)
     return dict(zip(keys, [int(v) for v in arr]))
 
 

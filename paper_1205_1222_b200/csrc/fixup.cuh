@@ -9,10 +9,10 @@
 // neighbour, so the result stays the sum over exactly the complement of the emitted list.  (A pair force_kernel took
 // on its far path is never a neighbour by that test either: the far threshold carries a 2^-10 margin, force.cuh.)
 //
-// Mapping: the queued rows are taken eight at a time (one row per warp); a work item is (group of 8 rows, j-chunk).
-// The 256 threads of a CTA predict a tile of 256 j straight from the registered fp64 state into shared memory (the
-// Horner form of predict.cuh; fp64 x_p, v_p, m and the fp32 record the neighbour test needs), then every warp runs its
-// row over the tile, lanes striding over j.  Lane sums are fp64, reduced by a fixed xor-shuffle tree; the chunks of a
+// Mapping: the queued rows are taken R at a time (R = 8, 4, 2 or 1: few rows -> all eight warps of a CTA on one row);
+// a work item is (group of R rows, j-chunk).  The 256 threads of a CTA predict a tile of 256 j straight from the
+// registered fp64 state into shared memory (the Horner form of predict.cuh; fp64 x_p, v_p, m and the fp32 record the
+// neighbour test needs), then every warp runs its row over its share of the tile, lanes striding over j.  Lane sums are fp64, reduced by a fixed xor-shuffle tree; the chunks of a
 // row are added in a fixed order by the CTA that finishes last (atomic ticket): deterministic for a given device.
 // The pass always runs (one launch); with nothing queued every CTA returns at once.
 #pragma once
@@ -47,14 +47,21 @@ template <bool VEL>
 __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
     __shared__ double sx[3][kFixThreads], sv[3][kFixThreads], sm[kFixThreads];
     __shared__ float sh[3][kFixThreads], sl[3][kFixThreads], sw[3][kFixThreads];
+    __shared__ double sred[kFixWarps][6];
     __shared__ int s_last;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    pdl_wait();
     const int32_t n_fix = *reinterpret_cast<volatile int32_t*>(a.count);
     if (n_fix == 0) {  // the usual case
         if (blockIdx.x == 0 && tid == 0) *a.stat_last = 0;
         return;
     }
-    const int32_t groups = (n_fix + kFixWarps - 1) / kFixWarps;
+    // Rows per CTA: a predicted tile serves up to eight rows, one per warp; with fewer than five rows queued (a small
+    // active block: the call is short and this pass must be too) the idle warps take a share of the tile instead.
+    // R is a function of n_fix alone: the same rows give the same bits.
+    const int R = n_fix >= 5 ? 8 : n_fix >= 3 ? 4 : n_fix == 2 ? 2 : 1;
+    const int nsub = kFixWarps / R, rs = warp % R, sub = warp / R;  // this warp: row slot, and which share of each tile
+    const int32_t groups = (n_fix + R - 1) / R;
     const int32_t n_tiles = (a.n + kFixThreads - 1) / kFixThreads;
     int32_t C = min(((int32_t)gridDim.x + groups - 1) / groups, n_tiles);  // j-chunks per group: enough items for the grid
     const int32_t tpc = (n_tiles + C - 1) / C;
@@ -63,7 +70,7 @@ __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
 
     for (int64_t item = blockIdx.x; item < items; item += gridDim.x) {
         const int32_t g = (int32_t)(item / C), c = (int32_t)(item % C);
-        const int32_t f = g * kFixWarps + warp;
+        const int32_t f = g * R + rs;
         const bool live = f < n_fix;  // warp-uniform
         // ---- this warp's row: predicted in fp64, and its fp32 record exactly as force_kernel's i-setup forms it
         int32_t orow = 0, i = 0;
@@ -87,8 +94,8 @@ __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
             I.nxh = -h[0]; I.nyh = -h[1]; I.nzh = -h[2];
             I.nxl = -l[0]; I.nyl = -l[1]; I.nzl = -l[2];
             I.nvx = -w[0]; I.nvy = -w[1]; I.nvz = -w[2];
-            const double rs = a.r_s[orow];
-            I.h2 = fmaxf(__double2float_rn(rs * rs), 1.17549435e-38f);
+            const double rs2 = a.r_s[orow];
+            I.h2 = fmaxf(__double2float_rn(rs2 * rs2), 1.17549435e-38f);
             I.dtr = VEL ? __double2float_rn(a.dtr[orow]) : 0.f;
         }
         double s[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
@@ -118,7 +125,7 @@ __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
             __syncthreads();
             if (!live) continue;
             const int32_t jn = min(kFixThreads, a.n - t * kFixThreads);
-            for (int32_t jj = lane; jj < jn; jj += 32) {
+            for (int32_t jj = sub * 32 + lane; jj < jn; jj += 32 * nsub) {
                 const int32_t j = t * kFixThreads + jj;
                 if (j == i) continue;
                 // the neighbour test of force_kernel's near path, on the same fp32 words (both halves hold j)
@@ -149,44 +156,50 @@ __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
                 s[5] += mri3 * (Vz + al * Rz);
             }
         }
+        // ---- the warp's lanes (fixed xor tree), then the warps that share the row (in order of their share)
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
 #pragma unroll
             for (int k = 0; k < 6; ++k) s[k] += __shfl_xor_sync(0xffffffffu, s[k], off);
         }
+        __syncthreads();  // sred of the previous item has been read
+        if (lane == 0) {
+#pragma unroll
+            for (int k = 0; k < 6; ++k) sred[warp][k] = s[k];
+        }
+        __syncthreads();
+        double v = 0.0;  // lanes 0-5 of the row's first warp: one component each
+        if (sub == 0 && lane < 6)
+            for (int u = 0; u < nsub; ++u) v += sred[rs + u * R][lane];
         if (C == 1) {
-            if (live && lane < 3) {
-                a.acc[(size_t)orow * 3 + lane] = (lane == 0) ? s[0] : (lane == 1) ? s[1] : s[2];
-                a.jerk[(size_t)orow * 3 + lane] = (lane == 0) ? s[3] : (lane == 1) ? s[4] : s[5];
+            if (live && sub == 0 && lane < 6) {
+                if (lane < 3) a.acc[(size_t)orow * 3 + lane] = v;
+                else a.jerk[(size_t)orow * 3 + lane - 3] = v;
             }
             continue;
         }
-        if (live && lane == 0) {
-            double* ps = a.part + ((size_t)item * kFixWarps + warp) * 6;
-#pragma unroll
-            for (int k = 0; k < 6; ++k) ps[k] = s[k];
-        }
+        if (live && sub == 0 && lane < 6) a.part[((size_t)item * kFixWarps + rs) * 6 + lane] = v;
         __threadfence();
         __syncthreads();
         if (tid == 0) s_last = (atomicAdd(a.tickets + g, 1) == C - 1);
         __syncthreads();
         if (s_last) {  // every chunk of this group is in: lanes stride over the chunks, then the fixed shuffle tree
             __threadfence();
-            if (live) {
-                double v[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+            if (live && sub == 0) {
+                double w[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
                 for (int32_t cc = lane; cc < C; cc += 32) {
-                    const double* ps = a.part + (((size_t)g * C + cc) * kFixWarps + warp) * 6;
+                    const double* ps = a.part + (((size_t)g * C + cc) * kFixWarps + rs) * 6;
 #pragma unroll
-                    for (int k = 0; k < 6; ++k) v[k] += __ldcg(ps + k);
+                    for (int k = 0; k < 6; ++k) w[k] += __ldcg(ps + k);
                 }
 #pragma unroll
                 for (int off = 16; off > 0; off >>= 1) {
 #pragma unroll
-                    for (int k = 0; k < 6; ++k) v[k] += __shfl_xor_sync(0xffffffffu, v[k], off);
+                    for (int k = 0; k < 6; ++k) w[k] += __shfl_xor_sync(0xffffffffu, w[k], off);
                 }
                 if (lane < 3) {
-                    a.acc[(size_t)orow * 3 + lane] = (lane == 0) ? v[0] : (lane == 1) ? v[1] : v[2];
-                    a.jerk[(size_t)orow * 3 + lane] = (lane == 0) ? v[3] : (lane == 1) ? v[4] : v[5];
+                    a.acc[(size_t)orow * 3 + lane] = (lane == 0) ? w[0] : (lane == 1) ? w[1] : w[2];
+                    a.jerk[(size_t)orow * 3 + lane] = (lane == 0) ? w[3] : (lane == 1) ? w[4] : w[5];
                 }
             }
             if (tid == 0) a.tickets[g] = 0;

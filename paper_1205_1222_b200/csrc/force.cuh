@@ -41,12 +41,14 @@ struct ForceArgs {
     RawState raw;           // PRED: the registered fp64 state and the time to predict to
     const float4* packed;   // packed j-pair records, n_pad / 2 pairs
     int32_t n;              // real j-particles
-    int32_t n_tiles;        // number of JT-sized tiles covering n_pad
+    int32_t n_pad;          // j-particles in the packed array (a multiple of kJPad; the padding is massless)
     // CTA b < main_blocks: row block b against the whole j-range, final outputs written directly.
     // CTA b >= main_blocks ("tail"): t = b - main_blocks, row block main_blocks + t / n_chunks against j-chunk
-    // t % n_chunks (tiles_per_chunk tiles), partial outputs for reduce_gather_kernel.
+    // t % n_chunks = particles [chunk * chunk_j, (chunk + 1) * chunk_j), partial outputs for reduce_gather_kernel
+    // (PAPER.md:122-126).  chunk_j is any multiple of 4 (not of the tile size): the planner cuts the j-range into
+    // exactly as many equal chunks as fill whole waves of CTA slots; a chunk's last tile is shorter than the others.
     int32_t main_blocks;
-    int32_t tiles_per_chunk;
+    int32_t chunk_j;
     int32_t n_chunks;       // S >= 2 for the tail blocks (unused when there is no tail)
     int32_t n_i;
     int32_t cap;
@@ -272,7 +274,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
     constexpr int kThreads = WARPS * 32;
     constexpr int kRows = kThreads * IPT;
     constexpr int kTileQuads = JT / 2 * kQuadsPerPair;
-    constexpr uint32_t kTileBytes = JT * kBytesPerJ;
+    constexpr uint32_t kTileBytes = JT * kBytesPerJ;  // a full tile; a chunk's last tile may be shorter
     constexpr int kStages = PRED ? 1 : 2;  // the fused-prediction variant fills its one stage itself
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -290,15 +292,16 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
 
     const int tid = threadIdx.x;
     const bool split = (int)blockIdx.x >= a.main_blocks;
-    int row_block = blockIdx.x, chunk = 0, t_begin = 0, t_end = a.n_tiles;
+    int row_block = blockIdx.x, chunk = 0;
+    int32_t j_begin = 0, j_end = a.n_pad;
     if (split) {
         const int t = blockIdx.x - a.main_blocks;
         row_block = a.main_blocks + t / a.n_chunks;
         chunk = t % a.n_chunks;
-        t_begin = chunk * a.tiles_per_chunk;
-        t_end = min(t_begin + a.tiles_per_chunk, a.n_tiles);
+        j_begin = chunk * a.chunk_j;
+        j_end = min(j_begin + a.chunk_j, a.n_pad);
     }
-    const int n_t = t_end - t_begin;
+    const int n_t = (j_end - j_begin + JT - 1) / JT;  // tiles of this CTA; the last one may be short (a multiple of 4 j)
     const int64_t tail_row0 = (int64_t)a.main_blocks * kRows;
 
     if (!PRED && tid == 0) {
@@ -306,9 +309,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         mbar_fence_init();
     }
     if (!PRED) __syncthreads();
+    pdl_wait();     // the predictor (or the row ordering) has finished; before this line nothing touched global memory
     if (!PRED && tid == 0 && n_t > 0) {  // prologue: first tile in flight while the i-state is gathered
-        mbar_arrive_expect_tx(&full[0], kTileBytes);
-        bulk_g2s(tiles, a.packed + (size_t)t_begin * kTileQuads, kTileBytes, &full[0]);
+        const uint32_t bytes = (uint32_t)min(JT, j_end - j_begin) * kBytesPerJ;
+        mbar_arrive_expect_tx(&full[0], bytes);
+        bulk_g2s(tiles, a.packed + (size_t)(j_begin >> 1) * kQuadsPerPair, bytes, &full[0]);
     }
 
     // ---- S2: i-setup.  Gather the active particles' predicted state from the packed records by index.
@@ -365,13 +370,17 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
     // ---- S3/S4: stream the j-tiles
     for (int lt = 0; lt < n_t; ++lt) {
         const int st = PRED ? 0 : (lt & 1);
+        const int32_t jbase = j_begin + lt * JT;             // first particle of this tile
+        const int32_t tile_j = min(JT, j_end - jbase);       // particles in it
         if (PRED) {  // predict this thread's j-pair of the tile into shared memory (layout of nbreg_common.cuh)
-            const int32_t j0 = (t_begin + lt) * JT + 2 * tid;
+            const int32_t j0 = jbase + 2 * tid;
             PredRecord r0, r1;
             r0.xh = r0.yh = r0.zh = kFarAway; r0.m = r0.xl = r0.yl = r0.zl = r0.vx = r0.vy = r0.vz = 0.f;
             r1 = r0;  // padding particles past n: massless, far away, at rest
-            if (j0 < a.n) r0 = predict_record(a.raw, j0);
-            if (j0 + 1 < a.n) r1 = predict_record(a.raw, j0 + 1);
+            if (2 * tid < tile_j) {  // (a short last tile: the other threads have nothing to predict)
+                if (j0 < a.n) r0 = predict_record(a.raw, j0);
+                if (j0 + 1 < a.n) r1 = predict_record(a.raw, j0 + 1);
+            }
             float4* o = tiles + tid * kQuadsPerPair;
             o[0] = make_float4(r0.xh, r1.xh, r0.yh, r1.yh);
             o[1] = make_float4(r0.zh, r1.zh, r0.m, r1.m);
@@ -381,23 +390,28 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
             if (WARPS > 1) __syncthreads(); else __syncwarp();
         }
         if (!PRED && tid == 0 && lt + 1 < n_t) {  // prefetch the next tile into the other stage (freed by the barrier below)
-            mbar_arrive_expect_tx(&full[st ^ 1], kTileBytes);
-            bulk_g2s(tiles + (st ^ 1) * kTileQuads, a.packed + (size_t)(t_begin + lt + 1) * kTileQuads, kTileBytes,
+            const uint32_t bytes = (uint32_t)min(JT, j_end - jbase - JT) * kBytesPerJ;
+            mbar_arrive_expect_tx(&full[st ^ 1], bytes);
+            bulk_g2s(tiles + (st ^ 1) * kTileQuads, a.packed + (size_t)((jbase + JT) >> 1) * kQuadsPerPair, bytes,
                      &full[st ^ 1]);
         }
         if (!PRED) mbar_wait(&full[st], (lt >> 1) & 1);
         const float4* tp = tiles + st * kTileQuads;
-        const int32_t jbase = (t_begin + lt) * JT;
         if (VEL) {  // far threshold of this tile: its fastest particle cannot bring a far pair within r_s during dtr
-            const float vmax = __ldg(a.tile_vmax + (jbase >> 8));
+            // (speed bounds are kept per 256 consecutive particles; a tile overlaps at most two such blocks)
+            const float vmax = fmaxf(__ldg(a.tile_vmax + (jbase >> 8)), __ldg(a.tile_vmax + ((jbase + tile_j - 1) >> 8)));
 #pragma unroll
             for (int u = 0; u < IPT; ++u) {
                 const float hf = fmaxf(I[u].hfar_x, fmaf(fabsf(I[u].dtr), vmax, I[u].hfar_r));
                 I[u].hfar2 = hf * hf;
             }
         }
-#pragma unroll 2
-        for (int p = 0; p < JT / 2; ++p) {
+        const int n_pp = tile_j >> 2;  // the tile's j-pairs, two per trip (tile_j is a multiple of 4)
+#pragma unroll 1
+        for (int pp = 0; pp < n_pp; ++pp) {
+#pragma unroll
+        for (int ph = 0; ph < 2; ++ph) {
+            const int p = 2 * pp + ph;
             const float4 q0 = tp[p * 5 + 0], q1 = tp[p * 5 + 1], q2 = tp[p * 5 + 2];
             const float2 vz = *reinterpret_cast<const float2*>(tp + p * 5 + 3);
             PairGeom g[IPT];
@@ -429,6 +443,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
             }
 #pragma unroll
             for (int u = 0; u < IPT; ++u) pair_sum<POT, false>(q1, q2, vz, I[u], g[u], s[u]);
+        }
         }
         // ---- S6: flush the tile's fp32 partial sums into the fp64 running sums
 #pragma unroll
@@ -463,6 +478,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
         }
         if (WARPS > 1) __syncthreads(); else __syncwarp();  // every warp is done with stage st before it is refilled
     }
+
+    pdl_trigger();  // the gather kernel may be scheduled once every CTA of this launch is through its j-loop
 
     // ---- outputs
 #pragma unroll

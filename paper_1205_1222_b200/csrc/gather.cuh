@@ -44,6 +44,7 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
     extern __shared__ int32_t stage_all[];  // kGatherWarps x (cap + S)
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
+    pdl_wait();
     const int64_t prow = (int64_t)blockIdx.x * kGatherWarps + warp;  // row among the split rows
     const int64_t row = a.row0 + prow;
     if (row < a.n_i) {  // warp-uniform
@@ -162,6 +163,7 @@ __global__ void __launch_bounds__(kWideThreadsFew) reduce_gather_wide_kernel(Gat
     __shared__ double row_sum[6];
     const int n_threads = blockDim.x;  // kWideThreads or kWideThreadsFew
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    pdl_wait();
     const int64_t prow = blockIdx.x;
     const int64_t lrow = a.row0 + prow;  // grid = split rows exactly
     const int64_t row = a.perm ? a.perm[lrow] : lrow;  // the caller's row

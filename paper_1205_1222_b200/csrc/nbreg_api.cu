@@ -47,6 +47,24 @@ namespace {
 
 thread_local char g_errbuf[256] = "";
 
+// Launch with the programmatic-stream-serialization attribute (nbreg_common.cuh: pdl_wait / pdl_trigger): the kernel may
+// be scheduled while the tail of the kernel before it is still running; it waits for that kernel's completion itself.
+bool g_pdl = true;  // "pdl" option of any context switches it for the process (a debugging aid)
+template <typename... KArgs, typename... Args>
+cudaError_t launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = g_pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+}
+
 int cuda_fail(cudaError_t e, const char* what) {
     snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error in %s: %s", what, cudaGetErrorString(e));
     return NB_E_CUDA;
@@ -71,11 +89,11 @@ constexpr Shape kShapes[kNumShapes] = {{256, 1, 8, 256}, {128, 1, 4, 256}, {64, 
 // and the j-split of the remaining ("tail") row blocks.
 struct Plan {
     int shape;          // index into kShapes
-    int n_tiles;        // j-tiles of kShapes[shape].jt covering n_pad
+    int n_pad;          // j-particles of the packed array (n rounded up to kJPad)
     int n_blocks;       // row blocks
     int main_blocks;    // row blocks handled by one CTA each
     int n_chunks;       // S: j-chunks per tail row block (1 = no tail: main_blocks == n_blocks)
-    int tiles_per_chunk;
+    int chunk_j;        // particles per chunk: a multiple of kChunkGrain, not of the tile size
     int grid;           // CTAs
     double cost;        // model cost in units of (one j against one CTA's rows)
 };
@@ -135,7 +153,7 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
     place((size_t)(n_i_max + 1) * sizeof(int32_t), w.fixrow_off, w.fixrow_bytes);
     place((size_t)(n_i_max + 1) * sizeof(float2), w.escale_off, w.escale_bytes);
     place((size_t)(n_i_max + 512) * sizeof(int32_t), w.slot_off, w.slot_bytes);
-    place((size_t)(n_i_max / kFixWarps + 2) * sizeof(int32_t), w.ftick_off, w.ftick_bytes);
+    place((size_t)(n_i_max / kFixWarps + 34) * sizeof(int32_t), w.ftick_off, w.ftick_bytes);
     place(128, w.ctl_off, w.ctl_bytes);
     w.total = off;
     return w;
@@ -206,6 +224,9 @@ constexpr int kWideGatherChunks = 64;
 constexpr int64_t kWideGatherRows = 4096;
 constexpr double kPrologueJ = 48.0;
 constexpr double kRaggedEnd = 0.2;
+constexpr int64_t kChunkGrain = 4;   // chunk lengths are multiples of this (the j-loop takes two j-pairs per trip)
+constexpr int64_t kMinChunkJ = 64;   // shortest chunk worth a CTA
+constexpr double kGatherJPerSlot = 0.0;  // gather cost per (row, chunk) partial sum, in j per CTA (calibrated below)
 
 struct Machine {
     int64_t n;        // j-particles
@@ -219,21 +240,26 @@ Plan plan_for_shape(const Machine* c, int32_t n_i, int shape, int64_t force_spli
     Plan p{};
     p.shape = shape;
     const int64_t n_pad = round_up(c->n, kJPad);
-    p.n_tiles = (int)(n_pad / sh.jt);
+    p.n_pad = (int)n_pad;
     p.n_blocks = (int)((n_i + sh.rows - 1) / sh.rows);
     const int64_t sms = c->num_sms > 0 ? c->num_sms : 148;
     const int64_t slots = sms * (c->ctas_per_sm[shape] > 0 ? c->ctas_per_sm[shape] : 1);
     const double t_full = kPrologueJ + (double)n_pad;
-    auto chunking = [&](int64_t S) {  // tiles per chunk and the resulting number of non-empty chunks
-        const int tpc = (int)((p.n_tiles + S - 1) / S);
-        return std::pair<int, int>(tpc, (p.n_tiles + tpc - 1) / tpc);
+    // S chunks of equal length (a multiple of kChunkGrain particles, whatever the tile size: a chunk's last tile is
+    // simply shorter), none empty
+    auto chunking = [&](int64_t S) {
+        const int64_t cj = std::max<int64_t>(kMinChunkJ, round_up((n_pad + S - 1) / S, kChunkGrain));
+        return std::pair<int, int>((int)cj, (int)((n_pad + cj - 1) / cj));
     };
     auto tail_cost = [&](int64_t tail, const std::pair<int, int>& ch) {
-        const double t = kPrologueJ + (double)ch.first * sh.jt;
+        const double t = kPrologueJ + (double)ch.first;
         const double waves = (double)(tail * ch.second) / (double)slots;
         // few waves run almost in lockstep (the count rounds up), many waves overlap freely
         const double eff_waves = std::max(1.0, 0.5 * std::ceil(waves) + 0.5 * waves);
-        return eff_waves * t + kRaggedEnd * t;
+        // ... plus what the gather kernel pays for the (row, chunk) partial sums it has to read: 64 B each at ~1.5 TB/s,
+        // in units of j per CTA (one j against a CTA's rows takes ~0.26 ns at 8 resident CTAs per SM)
+        const double gather = (double)(tail * sh.rows * ch.second) * kGatherJPerSlot;
+        return eff_waves * t + kRaggedEnd * t + gather;
     };
     int64_t tail = p.n_blocks, S = 1;
     if (force_split > 0) {
@@ -241,7 +267,7 @@ Plan plan_for_shape(const Machine* c, int32_t n_i, int shape, int64_t force_spli
     } else {
         tail = p.n_blocks % slots;
         if (tail > 0) {
-            int64_t s_max = std::min<int64_t>(p.n_tiles, c->row_chunk_limit / (tail * sh.rows));
+            int64_t s_max = std::min<int64_t>(n_pad / kMinChunkJ, c->row_chunk_limit / (tail * sh.rows));
             s_max = std::max<int64_t>(1, std::min<int64_t>(s_max, kMaxChunks));
             double best = 1e300;
             int last_chunks = 0;
@@ -258,14 +284,15 @@ Plan plan_for_shape(const Machine* c, int32_t n_i, int shape, int64_t force_spli
             }
         }
     }
-    if (S > p.n_tiles) S = p.n_tiles;
+    if (S > n_pad / kMinChunkJ) S = std::max<int64_t>(1, n_pad / kMinChunkJ);
     if (S > kMaxChunks) S = kMaxChunks;
     if (S > 1 && tail * sh.rows * S > c->row_chunk_limit) S = std::max<int64_t>(1, c->row_chunk_limit / (tail * sh.rows));
     const auto ch = chunking(S);
-    p.tiles_per_chunk = ch.first;
+    p.chunk_j = ch.first;
     p.n_chunks = ch.second;
     if (p.n_chunks <= 1) {
         p.n_chunks = 1;
+        p.chunk_j = (int)n_pad;
         tail = 0;
     }
     p.main_blocks = (int)(p.n_blocks - tail);
@@ -322,8 +349,7 @@ int query_force(int* per_sm) {
 template <int IPT, int WARPS, int JT, int MINB, bool VEL, bool POT>
 int launch_force(const Plan& p, const ForceArgs& fa, cudaStream_t st) {
     const size_t smem = force_smem_bytes(IPT, WARPS, JT, POT);
-    force_kernel<IPT, WARPS, JT, MINB, VEL, POT><<<p.grid, WARPS * 32, smem, st>>>(fa);
-    NB_CUDA(cudaGetLastError());
+    NB_CUDA(launch_k(force_kernel<IPT, WARPS, JT, MINB, VEL, POT>, p.grid, WARPS * 32, smem, st, fa));
     return NB_OK;
 }
 
@@ -338,8 +364,7 @@ int force_pred_dispatch(int shape, int* per_sm, const Plan* p, const ForceArgs* 
             NB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, WARPS * 32, smem));        \
             return NB_OK;                                                                                  \
         }                                                                                                  \
-        kern<<<p->grid, WARPS * 32, smem, st>>>(*fa);                                                      \
-        NB_CUDA(cudaGetLastError());                                                                       \
+        NB_CUDA(launch_k(kern, p->grid, WARPS * 32, smem, st, *fa));                                       \
         return NB_OK;                                                                                      \
     }
     switch (shape) {
@@ -392,13 +417,12 @@ int run_predict(nb_ctx* c, double t, cudaStream_t st, double* xp_out, double* vp
     if (xp_out) {
         const int64_t pairs = (c->n + 1) / 2;
         pa.n_pairs = pairs;
-        predict_kernel<true, false><<<(unsigned)((pairs + threads - 1) / threads), threads, 0, st>>>(pa);
+        NB_CUDA(launch_k(predict_kernel<true, false>, (unsigned)((pairs + threads - 1) / threads), threads, 0, st, pa));
     } else if (with_gather) {
-        predict_kernel<false, true><<<(unsigned)((pa.n_pairs + threads - 1) / threads), threads, 0, st>>>(pa);
+        NB_CUDA(launch_k(predict_kernel<false, true>, (unsigned)((pa.n_pairs + threads - 1) / threads), threads, 0, st, pa));
     } else {
-        predict_kernel<false, false><<<(unsigned)((pa.n_pairs + threads - 1) / threads), threads, 0, st>>>(pa);
+        NB_CUDA(launch_k(predict_kernel<false, false>, (unsigned)((pa.n_pairs + threads - 1) / threads), threads, 0, st, pa));
     }
-    NB_CUDA(cudaGetLastError());
     return NB_OK;
 }
 
@@ -630,9 +654,9 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     fa.raw = RawState{c->x0, c->v0, c->a0, c->j0, c->m, c->t0, t};
     fa.packed = reinterpret_cast<const float4*>(c->ws + c->lay.packed_off);
     fa.n = (int32_t)c->n;
-    fa.n_tiles = p.n_tiles;
+    fa.n_pad = p.n_pad;
     fa.main_blocks = p.main_blocks;
-    fa.tiles_per_chunk = p.tiles_per_chunk;
+    fa.chunk_j = p.chunk_j;
     fa.n_chunks = p.n_chunks;
     fa.n_i = n_i;
     fa.cap = c->cap;
@@ -649,10 +673,11 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     int32_t* ctl = reinterpret_cast<int32_t*>(c->ws + c->lay.ctl_off);
     // S2, first half: process the rows in Morton order of their predicted positions (order.cuh)
     fa.perm = nullptr;
-    // ... when the force kernel is long enough for the 2-7 % it gains to pay for the sort (~10 us in one CTA up to
-    // 8192 rows, ~60 us for the device-wide sort of larger blocks)
-    const double pairs = (double)n_i * (double)c->n;
-    const bool order_pays = n_i <= kSmallSort ? pairs >= 2.0e8 : pairs >= 1.0e9;
+    // ... when the force kernel is long enough for the 2-5 % it gains to pay for the sort (12-18 us in one CTA up to
+    // 8192 rows, ~60 us for the device-wide sort of larger blocks).  Measured break-even (A/B in one process, round 2):
+    // N = 65536: 8192 rows (5.4e8 pairs) -1 %, 16384 rows (1.1e9) +2 %; N = 2^20: 512 rows (5.4e8) -1 %, 1024 rows
+    // (1.1e9) +0.5 %, 8192 rows +3.4 %; N = 200000, 8192 rows (1.6e9) +1.6 %.
+    const bool order_pays = (double)n_i * (double)c->n >= 1.0e9;
     if (c->opt_order_rows == 2 || (c->opt_order_rows == 1 && n_i >= kOrderMinRows && order_pays)) {
         const size_t seg = (size_t)round_up((int64_t)std::max<int64_t>(c->n_i_max, 1) * 4, 256);
         unsigned char* sb = c->ws + c->lay.sort_off;
@@ -668,10 +693,9 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         oa.rows = reinterpret_cast<int32_t*>(sb + 2 * seg);
         if (n_i <= kSmallSort) {
             if (n_i <= 4096)
-                order_small_kernel<512, 8><<<1, 512, OrderSmall<512, 8>::smem_bytes, st>>>(oa);
+                NB_CUDA(launch_k(order_small_kernel<512, 8>, 1, 512, OrderSmall<512, 8>::smem_bytes, st, oa));
             else
-                order_small_kernel<1024, 8><<<1, 1024, OrderSmall<1024, 8>::smem_bytes, st>>>(oa);
-            NB_CUDA(cudaGetLastError());
+                NB_CUDA(launch_k(order_small_kernel<1024, 8>, 1, 1024, OrderSmall<1024, 8>::smem_bytes, st, oa));
             fa.perm = oa.rows;
             ++launches;
         } else {
@@ -707,7 +731,7 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         GatherArgs ga{};
         ga.row0 = (int32_t)(has_split ? row0 : n_i); ga.n_i = n_i; ga.n_chunks = p.n_chunks; ga.cap = c->cap;
         ga.perm = fa.perm;
-        ga.chunk_j = p.tiles_per_chunk * sh.jt;
+        ga.chunk_j = p.chunk_j;
         ga.part_sum = fa.part_sum;
         ga.fix = fa.fix;
         ga.acc = acc; ga.jerk = jerk; ga.pot = pot; ga.nbr_count = nbr_count; ga.nbr_list = nbr_list; ga.n_overflow = n_overflow;
@@ -715,13 +739,13 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         const int64_t split_rows = has_split ? n_i - row0 : 0;
         const unsigned blocks = (unsigned)std::max<int64_t>(1, (split_rows + kGatherWarps - 1) / kGatherWarps);
         if (has_split && p.n_chunks > kWideGatherChunks && split_rows <= kWideGatherRows) {  // few rows, many chunks
-            reduce_gather_wide_kernel<<<(unsigned)split_rows, split_rows <= kWideFewRows ? kWideThreadsFew : kWideThreads,
-                                        (size_t)c->cap * sizeof(int32_t), st>>>(ga);
+            NB_CUDA(launch_k(reduce_gather_wide_kernel, (unsigned)split_rows,
+                             split_rows <= kWideFewRows ? kWideThreadsFew : kWideThreads, (size_t)c->cap * sizeof(int32_t), st,
+                             ga));
         } else {
             const size_t stage = (size_t)kGatherWarps * (c->cap + p.n_chunks) * sizeof(int32_t);
-            reduce_gather_kernel<<<blocks, kGatherWarps * 32, stage, st>>>(ga);
+            NB_CUDA(launch_k(reduce_gather_kernel, blocks, kGatherWarps * 32, stage, st, ga));
         }
-        NB_CUDA(cudaGetLastError());
         ++launches;
     }
     if (c->opt_fixup) {  // fp64 fix-up of the rows the two kernels queued (usually none: every CTA returns at once)
@@ -737,9 +761,8 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         xa.stat_last = ctl + 18;
         xa.stat_total = reinterpret_cast<unsigned long long*>(ctl + 20);
         const unsigned grid = (unsigned)std::min(kFixMaxGrid, 2 * c->num_sms);
-        if (dtr) fixup_kernel<true><<<grid, kFixThreads, 0, st>>>(xa);
-        else fixup_kernel<false><<<grid, kFixThreads, 0, st>>>(xa);
-        NB_CUDA(cudaGetLastError());
+        if (dtr) NB_CUDA(launch_k(fixup_kernel<true>, grid, kFixThreads, 0, st, xa));
+        else NB_CUDA(launch_k(fixup_kernel<false>, grid, kFixThreads, 0, st, xa));
         ++launches;
     }
     c->info[0] = sh.rows; c->info[1] = sh.ipt; c->info[2] = p.n_chunks; c->info[3] = p.grid;
@@ -1075,6 +1098,11 @@ int nb_set_option(nb_ctx* c, const char* key, int64_t value) {
         c->opt_fuse_pred = value;
         return NB_OK;
     }
+    if (!strcmp(key, "pdl")) {
+        if (value > 1) return NB_E_INVAL;
+        g_pdl = value != 0;
+        return NB_OK;
+    }
     if (!strcmp(key, "gather_copy")) {
         if (value > 1) return NB_E_INVAL;
         c->opt_gather_copy = value;
@@ -1123,7 +1151,7 @@ int nb_plan(int64_t n, int32_t n_i, int32_t num_sms, const int32_t ctas_per_sm[5
     const Plan p = make_plan(&mach, n_i, i_block, j_split);
     const Shape& sh = kShapes[p.shape];
     info[0] = sh.rows; info[1] = sh.ipt; info[2] = p.n_chunks; info[3] = p.grid;
-    info[4] = p.n_blocks - p.main_blocks; info[5] = p.tiles_per_chunk; info[6] = sh.jt;
+    info[4] = p.n_blocks - p.main_blocks; info[5] = p.chunk_j; info[6] = sh.jt;
     info[7] = mach.ctas_per_sm[p.shape];
     return NB_OK;
 }

@@ -30,4 +30,21 @@ constexpr int kMaxNbrCap = 8192;       // nbr_cap limit: the gather kernel stage
 
 __host__ __device__ inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 
+// Programmatic dependent launch (sm_90+): the kernels of one call are launched with the programmatic-stream-
+// serialization attribute, so that a kernel's launch latency overlaps the tail of the kernel before it.  Every such
+// kernel calls pdl_wait() before it touches global memory (it returns once ALL earlier kernels of the stream have
+// completed and their writes are visible; a no-op for a kernel launched the ordinary way).  pdl_trigger() lets the next
+// kernel of the stream be scheduled once every CTA of this one has got that far (or has exited).  It sits LATE in the
+// kernels, after their main loop: CTAs of the next kernel that are resident while they wait take issue slots from the
+// CTAs still computing (measured: triggering at the start of force_kernel cost a 512-row call at N = 65536 14 %).
+#ifndef NBREG_PDL_TRIGGER
+#define NBREG_PDL_TRIGGER 1
+#endif
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() {
+#if NBREG_PDL_TRIGGER
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#endif
+}
+
 }  // namespace nbreg

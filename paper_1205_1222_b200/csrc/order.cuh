@@ -101,6 +101,7 @@ __global__ void __launch_bounds__(THREADS) order_small_kernel(OrderArgs a) {
     const int tid = threadIdx.x;
     if (tid < 6) box[tid] = 0u;
     __syncthreads();
+    pdl_wait();
     uint32_t m[6] = {0u, 0u, 0u, 0u, 0u, 0u};
     for (int q = tid; q < a.n_i; q += THREADS) {
         const float3 p = row_position(a, q);

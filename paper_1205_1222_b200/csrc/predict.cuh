@@ -45,6 +45,7 @@ __device__ __forceinline__ void load3(const double* base, int64_t j, double (&ou
 // decide that a far pair cannot come within r_s during dtr (force.cuh).
 template <bool WRITE_F64, bool GATHER>
 __global__ void __launch_bounds__(256) predict_kernel(PredictArgs a) {
+    pdl_wait();
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool active = p < a.n_pairs;
     const int64_t j0 = 2 * p;

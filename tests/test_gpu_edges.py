@@ -329,8 +329,12 @@ def test_host_entry_point_csr_lists(oracle, n, n_i):
     packed = csr["nbr_packed"].numpy()
     assert np.all(packed[total:] == -7)  # nothing written past the entries
     ref = dense["nbr_list"].numpy()
+    cnt = dense["nbr_count"].numpy()
     for q in range(0, wl.n_i, max(1, wl.n_i // 3000)):
-        assert np.array_equal(packed[off[q]:off[q + 1]], ref[q, : stored[q]])
+        if cnt[q] <= wl.cap:
+            assert np.array_equal(packed[off[q]:off[q + 1]], ref[q, : stored[q]])
+        else:  # an overflowed j-split row keeps cap of its neighbours, not necessarily the same ones in two runs (R7)
+            assert off[q + 1] - off[q] == wl.cap and np.all(np.diff(packed[off[q]:off[q + 1]]) > 0)
     if wl.n_i > 0:  # a buffer that is too small: NB_E_NOMEM, and the offsets say what is needed
         csr["nbr_packed"] = torch.empty(max(total // 2, 1), dtype=torch.int32)
         csr["nbr_offset"].fill_(-1)

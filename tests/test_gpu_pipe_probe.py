@@ -29,11 +29,14 @@ def test_packed_fp32_pipe_rates():
     r = json.loads(out)
     print("fp32x2 pipe probe:", r)
     nominal = r["nominal_lanes_per_clk_per_sm"]
-    for k in ("ffma2_3reg", "ffma2_shared", "fadd2", "fmul2", "mix", "mix_mufu", "ffma_scalar"):
+    keys = ("ffma2_3reg", "ffma2_shared", "fadd2", "fmul2", "fadd2_ffma2_1to1", "mix_6_6_13", "mix_6_6_13_shared",
+            "mix_6_6_13_mufu4", "mix_6_6_13_shared_mufu4", "ffma_scalar", "fadd_scalar", "mix_6_6_13_scalar")
+    for k in keys:
         assert 0.3 * nominal < r[k] <= 1.02 * nominal, (k, r[k])
-    # the two-operand packed instructions run near the nominal rate ...
-    assert r["fadd2"] > 0.9 * nominal and r["fmul2"] > 0.9 * nominal
-    # ... the kernel's mix with its MUFU share cannot be faster than the plain mix
-    assert r["mix_mufu"] <= r["mix"] * 1.01
+    # two-operand packed instructions come close to the nominal rate; FFMA2 with three distinct 64-bit register operands
+    # does not (register operand bandwidth): that is why the practical ceiling of the kernel's mix is below nominal
+    assert r["fadd2"] > 0.85 * nominal and r["fmul2"] > 0.85 * nominal
+    assert r["ffma2_3reg"] < r["ffma2_shared"] < 0.95 * nominal
+    assert r["mix_6_6_13_mufu4"] <= r["mix_6_6_13"] * 1.02
     if os.path.isdir(os.path.join(os.path.dirname(HERE), "gpurun_out")):
         json.dump(r, open(os.path.join(os.path.dirname(HERE), "gpurun_out", "pipe_probe.json"), "w"))

@@ -15,18 +15,17 @@ SHAPE = {256: 0, 128: 1, 64: 2, 32: 3, 512: 4}
 
 
 def _check_plan(p, n, n_i):
-    rows, jt = p["rows_per_cta"], p["j_tile"]
+    rows = p["rows_per_cta"]
     n_pad = (n + 255) // 256 * 256
-    n_tiles = n_pad // jt
     n_blocks = -(-n_i // rows)
     tail, S = p["split_row_blocks"], p["j_chunks"]
     assert 0 <= tail <= n_blocks and S >= 1
     assert (S == 1) == (tail == 0)
     assert p["ctas"] == (n_blocks - tail) + tail * S
     assert tail * rows * S <= min(max(256 * n_i, 131072), 2097152)  # (row, chunk) slots of the j-split workspace
-    if S > 1:  # the chunks cover the tiles exactly, none is empty
-        tpc = p["tiles_per_chunk"]
-        assert (S - 1) * tpc < n_tiles <= S * tpc
+    if S > 1:  # equal chunks (a multiple of 4 particles, not of the tile) cover the j-range exactly, none is empty
+        cj = p["chunk_j"]
+        assert cj % 4 == 0 and cj >= 64 and (S - 1) * cj < n_pad <= S * cj
     return n_blocks
 
 
@@ -47,7 +46,7 @@ def test_full_waves_run_unsplit_and_the_tail_fills_the_last_wave():
     # modelled time (in j per CTA slot) within 4 % of a perfectly balanced machine
     n_pad = 1 << 20
     waves_tail = -(-p["split_row_blocks"] * p["j_chunks"] // slots)
-    modelled = (n_blocks // slots) * n_pad + waves_tail * p["tiles_per_chunk"] * p["j_tile"]
+    modelled = (n_blocks // slots) * n_pad + waves_tail * p["chunk_j"]
     assert modelled <= 1.04 * n_blocks * n_pad / slots
     # an exact multiple of the slots needs no split at all
     q = binding.nb_plan(1 << 20, 444 * 256, 148, OCC, i_block=256)
@@ -60,17 +59,17 @@ def test_small_blocks_are_split_to_fill_the_machine():
         _check_plan(p, 65536, n_i)
         assert p["j_chunks"] > 1
         assert p["ctas"] >= 148  # at least one CTA per SM
-    # ... but never more chunks than j-tiles
+    # ... but no chunk shorter than 64 particles
     p = binding.nb_plan(300, 32, 148, OCC)
-    assert p["j_chunks"] <= 512 // p["j_tile"]
+    assert p["j_chunks"] <= 512 // 64
 
 
 def test_forced_options_are_honoured():
     for ib, sp in itertools.product((32, 64, 128, 256, 512), (1, 3, 7)):
         p = binding.nb_plan(2999, 777, 148, OCC, i_block=ib, j_split=sp)
         assert p["rows_per_cta"] == ib
-        n_tiles = 3072 // p["j_tile"]
-        want = -(-n_tiles // -(-n_tiles // sp))  # chunks are whole tiles and none is empty
+        cj = max(64, -(-(-(-3072 // sp)) // 4) * 4)   # equal chunks, a multiple of 4 particles, at least 64
+        want = -(-3072 // cj)                          # ... none empty
         assert p["j_chunks"] == want and (want == 1 or p["split_row_blocks"] == -(-777 // ib))
         _check_plan(p, 2999, 777)
     lib = binding.load()
