@@ -33,14 +33,15 @@ FLOPS_PER_PAIR = 60.0  # convention of BASELINE.json ("e.g. 60 for force+jerk"),
 # path = 25 of the SM's 128 FP32 lane-slots per pair.
 LANE_SLOTS_PER_PAIR = 25.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE force_kernel launch of the default workload, from the
-# committed capture profiles/r1_force_kernel_c5_ncu_full.md (ncu --set full); None for other workloads.
-FORCE_DRAM_BYTES_C5 = 1262.53e6 + 790.06e6
+# committed capture profiles/r2_force_kernel_c5_ncu_full.md (ncu --set full); None for other workloads.
+FORCE_DRAM_BYTES_C5 = 1450.77e6 + 945.16e6
 # algorithmic bytes of the predictor per particle on the regular-force path: 112 B of fp64 state read, 40 B of
 # pair-interleaved record written (the 48 B particle-major copy is written only for gathering consumers)
 PRED_BYTES_PER_J = 152
 # dram__bytes_read.sum + dram__bytes_write.sum of one predict_kernel launch of the default workload (ncu --set full,
-# profiles/r2_predict_kernel_c5_ncu_full.md); None until captured
-PRED_DRAM_BYTES_C5 = None
+# profiles/r2_force_kernel_c5_ncu_full.md): 117.45 MB read + 16.15 MB written -- less than the 159 MB the kernel moves,
+# because most of the 42 MB of records it writes are still in the 126 MB L2 when the capture ends
+PRED_DRAM_BYTES_C5 = 117.45e6 + 16.15e6
 METRIC = "regular-force Ginteractions/s (acc+jerk+nbr list)"
 UNIT = "Gpairs/s"
 
@@ -589,7 +590,7 @@ def run_gpu_arm(args):
                                "note": f"{PRED_BYTES_PER_J} B/j algorithmic (112 B of fp64 state read, 40 B pair record written; SURVEY "
                                        f"8(a) S1 budgets 112 + 48 = 160 B/j for a padded record: frac_at_survey_160_bytes), peak "
                                        f"{peaks['src']} copy bandwidth; ms is the interval between two events around ONE launch "
-                                       f"inside the step and includes the event-to-kernel latency (the kernel alone: "
+                                       f"inside the step and includes the event-to-kernel latency (the kernel alone, 24.8 us = 6.4 TB/s: "
                                        f"profiles/r2_bench_c5_launches.md)"},
         "launch": info, "gpu_launches": int(info["launches"] + 1) * args.steps,
         "fixup_rows_per_step": info["fixup_rows"],

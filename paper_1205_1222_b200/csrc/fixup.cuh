@@ -43,6 +43,23 @@ struct FixupArgs {
     unsigned long long* stat_total;  // [1] rows recomputed since nb_create
 };
 
+struct RawJ {  // one particle's registered fp64 state
+    double x[3], v[3], a[3], j[3], m, t0;
+};
+__device__ __forceinline__ RawJ load_raw(const RawState& r, int32_t j) {
+    RawJ w;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        w.x[k] = __ldg(r.x0 + 3 * (size_t)j + k);
+        w.v[k] = __ldg(r.v0 + 3 * (size_t)j + k);
+        w.a[k] = __ldg(r.a0 + 3 * (size_t)j + k);
+        w.j[k] = __ldg(r.j0 + 3 * (size_t)j + k);
+    }
+    w.m = __ldg(r.m + j);
+    w.t0 = __ldg(r.t0 + j);
+    return w;
+}
+
 template <bool VEL>
 __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
     __shared__ double sx[3][kFixThreads], sv[3][kFixThreads], sm[kFixThreads];
@@ -63,7 +80,9 @@ __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
     const int nsub = kFixWarps / R, rs = warp % R, sub = warp / R;  // this warp: row slot, and which share of each tile
     const int32_t groups = (n_fix + R - 1) / R;
     const int32_t n_tiles = (a.n + kFixThreads - 1) / kFixThreads;
-    int32_t C = min(((int32_t)gridDim.x + groups - 1) / groups, n_tiles);  // j-chunks per group: enough items for the grid
+    // j-chunks per group: as many items as fit ONE wave of the grid (a few more than the grid would make a second,
+    // almost empty wave: 63 groups x 5 chunks on 296 CTAs took twice as long as 63 x 4)
+    int32_t C = min(max((int32_t)gridDim.x / groups, 1), n_tiles);
     const int32_t tpc = (n_tiles + C - 1) / C;
     C = (n_tiles + tpc - 1) / tpc;
     const int64_t items = (int64_t)groups * C;
@@ -72,6 +91,12 @@ __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
         const int32_t g = (int32_t)(item / C), c = (int32_t)(item % C);
         const int32_t f = g * R + rs;
         const bool live = f < n_fix;  // warp-uniform
+        // the item's first tile: its loads are issued before the row's chain of dependent loads below, not after it
+        RawJ first{};
+        {
+            const int32_t j = c * tpc * kFixThreads + tid;
+            if (j < a.n) first = load_raw(a.raw, j);
+        }
         // ---- this warp's row: predicted in fp64, and its fp32 record exactly as force_kernel's i-setup forms it
         int32_t orow = 0, i = 0;
         double xi[3] = {0.0, 0.0, 0.0}, vi[3] = {0.0, 0.0, 0.0};
@@ -105,13 +130,12 @@ __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
             {
                 const int32_t j = t * kFixThreads + tid;
                 if (j < a.n) {
-                    const double dt = a.raw.t - __ldg(a.raw.t0 + j);
+                    const RawJ w = (t == c * tpc) ? first : load_raw(a.raw, j);
+                    const double dt = a.raw.t - w.t0;
 #pragma unroll
                     for (int k = 0; k < 3; ++k) {
-                        const double x = __ldg(a.raw.x0 + 3 * (size_t)j + k), v = __ldg(a.raw.v0 + 3 * (size_t)j + k);
-                        const double ac = __ldg(a.raw.a0 + 3 * (size_t)j + k), jk = __ldg(a.raw.j0 + 3 * (size_t)j + k);
-                        const double xp = x + dt * (v + dt * (0.5 * ac + dt * ((1.0 / 6.0) * jk)));
-                        const double vp = v + dt * (ac + dt * (0.5 * jk));
+                        const double xp = w.x[k] + dt * (w.v[k] + dt * (0.5 * w.a[k] + dt * ((1.0 / 6.0) * w.j[k])));
+                        const double vp = w.v[k] + dt * (w.a[k] + dt * (0.5 * w.j[k]));
                         const float xh = __double2float_rn(xp);
                         sx[k][tid] = xp;
                         sv[k][tid] = vp;
@@ -119,7 +143,7 @@ __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
                         sl[k][tid] = __double2float_rn(xp - (double)xh);
                         sw[k][tid] = __double2float_rn(vp);
                     }
-                    sm[tid] = __ldg(a.raw.m + j);
+                    sm[tid] = w.m;
                 }
             }
             __syncthreads();

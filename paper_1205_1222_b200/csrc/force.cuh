@@ -37,6 +37,13 @@ namespace nbreg {
 #endif
 constexpr float kFarFraction2 = NBREG_KAPPA2;
 
+// j-pairs per trip of the inner loop (unrolled), and the grain of a j-chunk's length that follows from it
+#ifndef NBREG_JUNROLL
+#define NBREG_JUNROLL 2
+#endif
+constexpr int kJUnroll = NBREG_JUNROLL;
+constexpr int kChunkGrain = 2 * kJUnroll;
+
 struct ForceArgs {
     RawState raw;           // PRED: the registered fp64 state and the time to predict to
     const float4* packed;   // packed j-pair records, n_pad / 2 pairs
@@ -406,12 +413,12 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {
                 I[u].hfar2 = hf * hf;
             }
         }
-        const int n_pp = tile_j >> 2;  // the tile's j-pairs, two per trip (tile_j is a multiple of 4)
+        const int n_pp = tile_j / (2 * kJUnroll);  // the tile's j-pairs, kJUnroll per trip (tile_j is a multiple of kChunkGrain)
 #pragma unroll 1
         for (int pp = 0; pp < n_pp; ++pp) {
 #pragma unroll
-        for (int ph = 0; ph < 2; ++ph) {
-            const int p = 2 * pp + ph;
+        for (int ph = 0; ph < kJUnroll; ++ph) {
+            const int p = kJUnroll * pp + ph;
             const float4 q0 = tp[p * 5 + 0], q1 = tp[p * 5 + 1], q2 = tp[p * 5 + 2];
             const float2 vz = *reinterpret_cast<const float2*>(tp + p * 5 + 3);
             PairGeom g[IPT];

@@ -224,7 +224,6 @@ constexpr int kWideGatherChunks = 64;
 constexpr int64_t kWideGatherRows = 4096;
 constexpr double kPrologueJ = 48.0;
 constexpr double kRaggedEnd = 0.2;
-constexpr int64_t kChunkGrain = 4;   // chunk lengths are multiples of this (the j-loop takes two j-pairs per trip)
 constexpr int64_t kMinChunkJ = 64;   // shortest chunk worth a CTA
 constexpr double kGatherJPerSlot = 0.0;  // gather cost per (row, chunk) partial sum, in j per CTA (calibrated below)
 
