@@ -462,6 +462,24 @@ def run_gpu_arm(args):
     value = whole_job_rate(job_pairs, args.steps, job_replicas, t_max)
     n_over = int(out["n_overflow"].item())
     mean_cnt = float(out["nbr_count"].double().mean().item())
+    # the predictor alone: ten launches back to back between two events (one launch inside the step is 25 us of kernel
+    # behind ~15 us of event-to-kernel latency, which says nothing about the kernel).  State + records = 159 MB > L2.
+    # Replayed from a CUDA graph, so that the host's enqueue rate (two ctypes calls per launch) is not what is timed.
+    pgraph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(pgraph):
+        for _ in range(10):
+            ctx.nb_predict_j(s.t)
+    pgraph.replay()
+    pe = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    flush.fill_(1)
+    torch.cuda.synchronize()
+    pe[0].record()
+    pgraph.replay()
+    pe[1].record()
+    torch.cuda.synchronize()
+    t_pred_b2b = pe[0].elapsed_time(pe[1]) / 10 / 1e3
+    del pgraph
+    ctx.nb_set_j(*state_dev)
 
     # ---- the step on the other side of the neighbour list: irregular force eq. (7), (8) over the
     # lists the last step produced.  Reported beside the headline, not part of it.
@@ -583,14 +601,17 @@ def run_gpu_arm(args):
                              f"file holds no FP32 figure, DESIGN.md section 7 derives this one); fma_pipe_busy = "
                              f"{LANE_SLOTS_PER_PAIR:.0f} issued FP32 lane-slots per pair / 128 per clock per SM",
                      "ms": t_force * 1e3},
-        "roofline_predictor": {"bound": "hbm", "kernel": "predict_kernel", "achieved": pred_bytes / t_pred / 1e9,
-                               "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": pred_bytes / t_pred / 1e9 / peaks["hbm_gbs"],
-                               "frac_at_survey_160_bytes": s.n * 160 / t_pred / 1e9 / peaks["hbm_gbs"],
-                               "traffic": PRED_DRAM_BYTES_C5 if headline else None, "ms": t_pred * 1e3,
+        "roofline_predictor": {"bound": "hbm", "kernel": "predict_kernel", "achieved": pred_bytes / t_pred_b2b / 1e9,
+                               "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": pred_bytes / t_pred_b2b / 1e9 / peaks["hbm_gbs"],
+                               "frac_at_survey_160_bytes": s.n * 160 / t_pred_b2b / 1e9 / peaks["hbm_gbs"],
+                               "traffic": PRED_DRAM_BYTES_C5 if headline else None, "ms": t_pred_b2b * 1e3,
+                               "ms_inside_step": t_pred * 1e3,
                                "note": f"{PRED_BYTES_PER_J} B/j algorithmic (112 B of fp64 state read, 40 B pair record written; SURVEY "
                                        f"8(a) S1 budgets 112 + 48 = 160 B/j for a padded record: frac_at_survey_160_bytes), peak "
-                                       f"{peaks['src']} copy bandwidth; ms is the interval between two events around ONE launch "
-                                       f"inside the step and includes the event-to-kernel latency (the kernel alone, 24.8 us = 6.4 TB/s: "
+                                       f"{peaks['src']} copy bandwidth; ms = average of ten launches back to back (one CUDA-graph replay) between two "
+                                       f"CUDA events (L2 flushed before; state + records exceed the L2); ms_inside_step = the interval between "
+                                       f"two events around the ONE launch of a timed step, which includes the event-to-kernel "
+                                       f"latency (the kernel alone under ncu, cold: 24.8 us = 6.4 TB/s, "
                                        f"profiles/r2_bench_c5_launches.md)"},
         "launch": info, "gpu_launches": int(info["launches"] + 1) * args.steps,
         "fixup_rows_per_step": info["fixup_rows"],

@@ -102,7 +102,8 @@ int nb_get_predicted(nb_ctx* ctx, double* xp, double* vp, void* stream);
  *   nbr_list:   dev int32[n_i][nbr_cap]  row q valid in [0, min(count, nbr_cap)), ascending j; the self index
  *               is never listed or counted; entries past the count are left untouched.  An overflowed row
  *               (count > nbr_cap) holds nbr_cap of its neighbours: the first ones in j if the row ran in one
- *               CTA, otherwise whichever reserved a slot first (reading R7/R15 in DESIGN.md)
+ *               CTA, otherwise whichever reserved a slot first -- which may differ between two runs -- unless option
+ *               "ovf_first_in_j" is set (reading R7/R15 in DESIGN.md)
  *   n_overflow: dev int32[1]     number of rows with count > nbr_cap
  * The pair within 1e-6 (relative) of r_s may fall on either side of the test (fp32 squares). */
 int nb_regular_force(nb_ctx* ctx, int32_t n_i, const int32_t* i_idx, const double* r_s, double t, double* acc,
@@ -250,6 +251,15 @@ int nb_fixup_stats(nb_ctx* ctx, int64_t stats[2], void* stream);
  *   "irr_pred"  how nb_irregular_force gets its predicted particles when the context holds no prediction at t:
  *               0 (default): rows <= n / 96 predict what they gather (as nb_irregular_force_act), larger blocks
  *               predict all n first; 1: always predict all; 2: always fused.  Results are identical bit for bit
+ *   "gather_copy" 0 (default): the predictor writes the particle-major copy of the records (for nb_irregular_force and
+ *               nb_regular_correct) only from the first such call of the context on; 1: from the start
+ *   "fixup", "fixup_ca_milli", "fixup_cj_milli": the fp64 fix-up pass, see nb_get_error_scale above
+ *   "ovf_first_in_j" 0 (default): an overflowed row whose j-range was split over several CTAs keeps whichever nbr_cap
+ *               neighbours reserved a list slot first (may differ from run to run); 1: one more kernel rewrites the lists
+ *               of such rows as the FIRST nbr_cap neighbours in ascending j, as rows run by one CTA keep them anyway:
+ *               reproducible lists, at ~n/32 warp iterations per overflowed row
+ *   "pdl"       1 (default): the kernels of a call are chained by programmatic dependent launch; 0: ordinary launches
+ *               (process-wide; a debugging aid)
  * Returns NB_E_INVAL for an unknown key or value. */
 int nb_set_option(nb_ctx* ctx, const char* key, int64_t value);
 

@@ -21,14 +21,22 @@ struct FixupFlag {
     int32_t* count;   // [1] rows queued so far in this call (zero between calls: fixup_kernel consumes and re-zeroes it)
     int32_t* rows;    // [n_i_max] the caller's rows that were queued, in arrival order
     float2* escale;   // [n_i_max] per caller's row: (sum_T |acc_T|^2, sum_T |jerk_T|^2), kept for nb_get_error_scale
-    float ca2, cj2;   // a row is queued iff ca2 * qa > |acc|^2 or cj2 * qj > |jerk|^2 (both 0: never)
+    float ca2, cj2;   // C_a^2, C_j^2 (both 0: never queue)
+    float inv_tiles;  // 1 / (number of j-tiles a row's sums were flushed from)
 };
 
+// q = sum_T |p_T|^2 over the T tile partials p_T of a row, whose sum is s.  The part of q that is NOT error scale is the
+// coherent one: if every tile contributed its share s / T, q would be |s|^2 / T (a smooth field; it dominates when there
+// are few tiles).  What is left, q - |s|^2 / T = sum_T |p_T - s / T|^2, estimates sum_j |term_j|^2.  A row is queued iff
+//     C^2 (q - |s|^2 / T) > |s|^2,   i.e.   C^2 q > |s|^2 (1 + C^2 / T),
+// for acc or for jerk.
 __device__ __forceinline__ void fixup_flag(const FixupFlag& f, int32_t orow, float qa, float qj, double ax, double ay,
                                            double az, double jx, double jy, double jz) {
     f.escale[orow] = make_float2(qa, qj);
     const double a2 = ax * ax + ay * ay + az * az, j2 = jx * jx + jy * jy + jz * jz;
-    if ((double)f.ca2 * (double)qa > a2 || (double)f.cj2 * (double)qj > j2) f.rows[atomicAdd(f.count, 1)] = orow;
+    const double ca2 = f.ca2, cj2 = f.cj2, it = f.inv_tiles;
+    if (ca2 * (double)qa > a2 * (1.0 + ca2 * it) || cj2 * (double)qj > j2 * (1.0 + cj2 * it))
+        f.rows[atomicAdd(f.count, 1)] = orow;
 }
 
 }  // namespace nbreg

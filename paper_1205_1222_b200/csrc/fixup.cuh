@@ -242,4 +242,95 @@ __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// Option "ovf_first_in_j": a reproducible list for overflowed j-split rows.
+//
+// The list of a row keeps nbr_cap of its neighbours when it overflows (reading R7).  A row one CTA ran over the whole
+// j-range keeps the first nbr_cap in ascending j; the CTAs of a j-split row reserve list slots with an atomic, so WHICH
+// nbr_cap neighbours it keeps depends on the order in which they arrive and can differ from run to run (the paper's
+// ring buffer at least is deterministic, PAPER.md:383-388, and PAPER.md:203 cares about reproducibility).  With the
+// option on, the gather kernels queue the overflowed j-split rows and this kernel rewrites their lists: one warp per
+// row walks the j-particles in ascending order, 32 at a time, repeats force_kernel's fp32 neighbour test (the same
+// device functions on the same fp32 records: the packed records if the context holds a prediction, else predicted on
+// the spot), and compacts the hits with ballot + popc until nbr_cap entries are stored.  Counts, overflow flag and forces
+// are untouched.  Off by default: overflow is the exception (the caller sizes nbr_cap), and the walk costs a warp
+// ~N / 32 iterations per overflowed row.
+struct OverflowListArgs {
+    RawState raw;
+    const float4* packed;      // pair-interleaved predicted records, or null: predict from raw
+    int32_t n;
+    int32_t cap;
+    const int32_t* i_idx;
+    const double* r_s;
+    const double* dtr;         // VEL, else null
+    int32_t* nbr_list;
+    int32_t* count;            // [1] queued rows (zero between calls; re-zeroed here)
+    const int32_t* rows;       // [count] caller's rows
+    int32_t* done;             // [1] CTAs of this launch that are done (zero between calls)
+};
+
+constexpr int kOvfWarps = 4;
+
+template <bool VEL>
+__global__ void __launch_bounds__(kOvfWarps * 32) overflow_list_kernel(OverflowListArgs a) {
+    const int lane = threadIdx.x & 31;
+    pdl_wait();
+    const int32_t n_rows = *reinterpret_cast<volatile int32_t*>(a.count);
+    if (n_rows == 0) return;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    for (int32_t f = blockIdx.x * kOvfWarps + (threadIdx.x >> 5); f < n_rows; f += gridDim.x * kOvfWarps) {
+        const int32_t orow = a.rows[f];
+        const int32_t i = a.i_idx[orow];
+        auto record = [&](int32_t j) {
+            if (!a.packed) return predict_record(a.raw, j);
+            const float* rec = reinterpret_cast<const float*>(a.packed + (size_t)(j >> 1) * kQuadsPerPair) + (j & 1);
+            PredRecord r;
+            r.xh = __ldg(rec); r.yh = __ldg(rec + 2); r.zh = __ldg(rec + 4); r.m = 0.f;
+            r.vx = __ldg(rec + 8); r.vy = __ldg(rec + 10); r.vz = __ldg(rec + 12);
+            r.xl = __ldg(rec + 14); r.yl = __ldg(rec + 16); r.zl = __ldg(rec + 18);
+            return r;
+        };
+        const PredRecord ri = record(i);
+        IState I{};
+        I.nxh = -ri.xh; I.nyh = -ri.yh; I.nzh = -ri.zh;
+        I.nxl = -ri.xl; I.nyl = -ri.yl; I.nzl = -ri.zl;
+        I.nvx = -ri.vx; I.nvy = -ri.vy; I.nvz = -ri.vz;
+        const double rs = a.r_s[orow];
+        I.h2 = fmaxf(__double2float_rn(rs * rs), 1.17549435e-38f);
+        I.dtr = VEL ? __double2float_rn(a.dtr[orow]) : 0.f;
+        int32_t* list = a.nbr_list + (size_t)orow * a.cap;
+        int32_t pos = 0;
+        for (int32_t base = 0; base < a.n && pos < a.cap; base += 32) {
+            const int32_t j = base + lane;
+            bool nb = false;
+            if (j < a.n && j != i) {
+                const PredRecord rj = record(j);
+                const float4 q0 = make_float4(rj.xh, rj.xh, rj.yh, rj.yh);
+                const float4 q1 = make_float4(rj.zh, rj.zh, 0.f, 0.f);
+                const float4 q2 = make_float4(rj.vx, rj.vx, rj.vy, rj.vy);
+                const float2 vz = make_float2(rj.vz, rj.vz);
+                const float2 xl = make_float2(rj.xl, rj.xl);
+                const float4 q4 = make_float4(rj.yl, rj.yl, rj.zl, rj.zl);
+                PairGeom gm;
+                geom_hi(q0, q1, I, gm);
+                geom_lo(xl, q4, I, gm);
+                const float2 rm = VEL ? rmin2_velocity(q2, vz, I, gm) : gm.r2;
+                nb = rm.x < I.h2;
+            }
+            const uint32_t hits = __ballot_sync(0xffffffffu, nb);
+            const int32_t at = pos + __popc(hits & lt_mask);
+            if (nb && at < a.cap) list[at] = j;
+            pos += __popc(hits);
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(a.done, 1) == (int32_t)gridDim.x - 1) {
+            *a.count = 0;
+            *a.done = 0;
+        }
+    }
+}
+
 }  // namespace nbreg

@@ -36,6 +36,10 @@ struct GatherArgs {
     int32_t* slot_count;       // [split rows] true counts of the j-split rows, complete when this kernel starts
     int32_t* overflow_ws;      // [1]
     int32_t* ticket;           // [1] blocks of this kernel that are done
+    // option "ovf_first_in_j": overflowed j-split rows are queued for overflow_list_kernel (fixup.cuh), which rewrites
+    // their lists as the first cap neighbours in ascending j (null: off)
+    int32_t* ovf_count;        // [1] (zero between calls)
+    int32_t* ovf_rows;         // [n_i_max] caller's rows
 };
 
 constexpr int kGatherWarps = 4;
@@ -128,7 +132,10 @@ __global__ void __launch_bounds__(kGatherWarps * 32) reduce_gather_kernel(Gather
         if (valid && before == 0) bin[c] += __popc(peers);
         __syncwarp();
     }
-    if (lane == 0 && cnt > a.cap) atomicAdd(a.overflow_ws, 1);
+    if (lane == 0 && cnt > a.cap) {
+        atomicAdd(a.overflow_ws, 1);
+        if (a.ovf_rows) a.ovf_rows[atomicAdd(a.ovf_count, 1)] = (int32_t)orow;
+    }
     }  // row < n_i
 
     // ---- the last block to finish publishes the overflow count of the whole call and re-zeroes the scratch
@@ -217,7 +224,10 @@ __global__ void __launch_bounds__(kWideThreadsFew) reduce_gather_wide_kernel(Gat
     if (tid == 0) {
         a.nbr_count[row] = cnt;
         a.slot_count[prow] = 0;
-        if (cnt > a.cap) atomicAdd(a.overflow_ws, 1);
+        if (cnt > a.cap) {
+            atomicAdd(a.overflow_ws, 1);
+            if (a.ovf_rows) a.ovf_rows[atomicAdd(a.ovf_count, 1)] = (int32_t)row;
+        }
         float qa = 0.f, qj = 0.f;
         for (int w = 0; w < n_threads / 32; ++w) {  // fixed order
             qa += warp_q[w].x;

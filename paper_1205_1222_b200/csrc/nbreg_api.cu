@@ -107,6 +107,7 @@ struct WorkspaceLayout {
     size_t sort_temp_bytes;
     size_t fixrow_off, fixrow_bytes;  // int32 caller's rows queued for the fp64 fix-up pass (fixup.cuh)
     size_t escale_off, escale_bytes;  // float2 error scales per caller's row (fixflag.cuh)
+    size_t ovfrow_off, ovfrow_bytes;  // int32 caller's rows queued for overflow_list_kernel (option "ovf_first_in_j")
     size_t slot_off, slot_bytes;   // int32 list-slot counters of the j-split rows (zero between calls)
     size_t ftick_off, ftick_bytes; // int32 chunk tickets of the fix-up groups (zero between calls)
     // int32 {overflow count, gather ticket, order ticket, -, 6 box words, -, -, -, -, -, -, fix-up queue length, fix-up
@@ -152,6 +153,7 @@ WorkspaceLayout layout(int64_t n_max, int64_t n_i_max, int32_t cap) {
     }
     place((size_t)(n_i_max + 1) * sizeof(int32_t), w.fixrow_off, w.fixrow_bytes);
     place((size_t)(n_i_max + 1) * sizeof(float2), w.escale_off, w.escale_bytes);
+    place((size_t)(n_i_max + 1) * sizeof(int32_t), w.ovfrow_off, w.ovfrow_bytes);
     place((size_t)(n_i_max + 512) * sizeof(int32_t), w.slot_off, w.slot_bytes);
     place((size_t)(n_i_max / kFixWarps + 34) * sizeof(int32_t), w.ftick_off, w.ftick_bytes);
     place(128, w.ctl_off, w.ctl_bytes);
@@ -195,6 +197,7 @@ struct nb_ctx {
     // fp64 fix-up of cancellation-dominated rows (fixflag.cuh): a row is recomputed iff C_a sqrt(q_a) > |acc| or
     // C_j sqrt(q_j) > |jerk|; the options hold 1000 C_a and 1000 C_j
     int64_t opt_fixup = 1, opt_fix_ca_milli = kFixCaMilli, opt_fix_cj_milli = kFixCjMilli;
+    int64_t opt_ovf_first = 0;  // overflowed j-split rows keep the first nbr_cap neighbours in j (overflow_list_kernel)
     // last launch
     int64_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     // host path: device mirrors owned by the context
@@ -721,6 +724,10 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         const float cj = c->opt_fixup ? 1e-3f * (float)c->opt_fix_cj_milli : 0.f;
         fa.fix.ca2 = ca * ca;
         fa.fix.cj2 = cj * cj;
+        // rows run by one CTA over the whole j-range.  (One tile says nothing about the spread of the terms: inv_tiles = 0
+        // then queues every row -- such a system is a few hundred particles, fp64 costs nothing.)
+        const int64_t tiles_main = (p.n_pad + sh.jt - 1) / sh.jt;
+        fa.fix.inv_tiles = tiles_main > 1 ? 1.0f / (float)tiles_main : 0.f;
     }
     int rc = fuse_pred ? force_pred_dispatch(p.shape, nullptr, &p, &fa, st)
                        : force_dispatch(variant, p.shape, nullptr, &p, &fa, st);
@@ -733,8 +740,13 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         ga.chunk_j = p.chunk_j;
         ga.part_sum = fa.part_sum;
         ga.fix = fa.fix;
+        ga.fix.inv_tiles = 1.0f / (float)((int64_t)p.n_chunks * ((p.chunk_j + sh.jt - 1) / sh.jt));  // j-split rows
         ga.acc = acc; ga.jerk = jerk; ga.pot = pot; ga.nbr_count = nbr_count; ga.nbr_list = nbr_list; ga.n_overflow = n_overflow;
         ga.slot_count = fa.slot_count; ga.overflow_ws = ctl; ga.ticket = ctl + 1;
+        if (c->opt_ovf_first) {
+            ga.ovf_count = ctl + 24;
+            ga.ovf_rows = reinterpret_cast<int32_t*>(c->ws + c->lay.ovfrow_off);
+        }
         const int64_t split_rows = has_split ? n_i - row0 : 0;
         const unsigned blocks = (unsigned)std::max<int64_t>(1, (split_rows + kGatherWarps - 1) / kGatherWarps);
         if (has_split && p.n_chunks > kWideGatherChunks && split_rows <= kWideGatherRows) {  // few rows, many chunks
@@ -745,6 +757,19 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
             const size_t stage = (size_t)kGatherWarps * (c->cap + p.n_chunks) * sizeof(int32_t);
             NB_CUDA(launch_k(reduce_gather_kernel, blocks, kGatherWarps * 32, stage, st, ga));
         }
+        ++launches;
+    }
+    if (c->opt_ovf_first && has_split) {  // reproducible lists for overflowed j-split rows (fixup.cuh)
+        OverflowListArgs oa{};
+        oa.raw = fa.raw;
+        oa.packed = fuse_pred ? nullptr : fa.packed;
+        oa.n = (int32_t)c->n; oa.cap = c->cap;
+        oa.i_idx = i_idx; oa.r_s = r_s; oa.dtr = dtr;
+        oa.nbr_list = nbr_list;
+        oa.count = ctl + 24; oa.rows = reinterpret_cast<int32_t*>(c->ws + c->lay.ovfrow_off); oa.done = ctl + 25;
+        const unsigned grid = (unsigned)(2 * c->num_sms);
+        if (dtr) NB_CUDA(launch_k(overflow_list_kernel<true>, grid, kOvfWarps * 32, 0, st, oa));
+        else NB_CUDA(launch_k(overflow_list_kernel<false>, grid, kOvfWarps * 32, 0, st, oa));
         ++launches;
     }
     if (c->opt_fixup) {  // fp64 fix-up of the rows the two kernels queued (usually none: every CTA returns at once)
@@ -1105,6 +1130,11 @@ int nb_set_option(nb_ctx* c, const char* key, int64_t value) {
     if (!strcmp(key, "gather_copy")) {
         if (value > 1) return NB_E_INVAL;
         c->opt_gather_copy = value;
+        return NB_OK;
+    }
+    if (!strcmp(key, "ovf_first_in_j")) {
+        if (value > 1) return NB_E_INVAL;
+        c->opt_ovf_first = value;
         return NB_OK;
     }
     if (!strcmp(key, "fixup")) {

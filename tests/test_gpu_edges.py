@@ -300,6 +300,34 @@ def test_host_entry_point_in_row_chunks(oracle):
     ctx.close()
 
 
+@pytest.mark.parametrize("fuse", [0, 2])
+def test_overflowed_split_rows_keep_the_first_cap_in_j_on_request(oracle, fuse):
+    """Option "ovf_first_in_j": the list of an overflowed j-split row is rewritten as the first nbr_cap neighbours in
+    ascending j (what a row run by one CTA keeps anyway): equal to the head of the oracle's list, and identical in two
+    runs.  fuse = 2: the call predicts inside the force kernel, the rewrite predicts what it tests."""
+    wl = _wl(oracle, 6000, 200, 20, 32)
+    wl.r_s[::7] *= 2.5  # ~300 neighbours > cap 32 on every 7th row
+    xp, vp = oracle.predict_state(wl.state)
+    _, _, cnt_o, lists_o = oracle.regular_force(xp, vp, wl.state.m, wl.i_idx, wl.r_s, list_stride=1024)
+    opts = {"ovf_first_in_j": 1, "i_block": 64, "j_split": 9, "fuse_pred": fuse}
+    g1, info = run_gpu(wl, options=opts)
+    g2, _ = run_gpu(wl, options=opts)
+    assert info["j_chunks"] == 9 and int(g1["n_overflow"][0]) >= 25
+    over = np.nonzero(g1["nbr_count"] > wl.cap)[0]
+    assert len(over) == int(g1["n_overflow"][0])
+    for q in over:
+        assert np.array_equal(g1["nbr_list"][q], lists_o[q][: wl.cap]), q      # the first cap in ascending j
+        assert np.array_equal(g1["nbr_list"][q], g2["nbr_list"][q])
+    assert np.array_equal(g1["nbr_count"], cnt_o)
+    _full_check(oracle, wl, g1)
+    # ... and with the velocity criterion
+    dtr = np.full(wl.n_i, 1.0 / 64)
+    g3, _ = run_gpu(wl, options={"ovf_first_in_j": 1, "i_block": 64, "j_split": 9}, dtr=dtr)
+    _, _, _, cnt_v, lists_v = oracle.regular_force_ex(xp, vp, wl.state.m, wl.i_idx, wl.r_s, dtr, list_stride=1024)
+    for q in np.nonzero(g3["nbr_count"] > wl.cap)[0]:
+        assert np.array_equal(g3["nbr_list"][q], lists_v[q][: wl.cap]), q
+
+
 @pytest.mark.parametrize("n,n_i", [(3001, 257), (2500, 40001), (900, 0)])
 def test_host_entry_point_csr_lists(oracle, n, n_i):
     """nb_regular_force_host_csr: the same outputs with the lists packed back to back (CSR), in one chunk and in several
