@@ -992,8 +992,10 @@ static int regular_force_host_impl(nb_ctx* c, int64_t n, const double* x0, const
     // ... when that pays: a row costs ~N ns of compute per 1000 j and (4 cap + 52) B of copy at ~50 GB/s (dense lists;
     // ~4 x 100 + 60 B in CSR form); splitting a block costs a few per cent of kernel efficiency, so it is done only if
     // the copy is >= 10 % of the compute
+    // (CSR form: a row is ~460 B; every row chunk also costs its own launches, a scan and a host synchronisation, so the
+    // copy must be a quarter of the compute before chunks pay: config 3 in 4 chunks 5.16 ms, in one 4.8 ms)
     const double row_bytes = csr ? 460.0 : (double)(4 * (int64_t)c->cap + 52);
-    const bool overlap_pays = row_bytes / 50.0 >= 0.1 * (double)n / 1000.0;
+    const bool overlap_pays = row_bytes / 50.0 >= (csr ? 0.25 : 0.1) * (double)n / 1000.0;
     int64_t rows_per_chunk = std::max<int64_t>(kHostChunkMinRows, (n_i + kHostChunks - 1) / kHostChunks);
     rows_per_chunk = round_up(rows_per_chunk, 1024);
     if (!overlap_pays) rows_per_chunk = round_up(std::max<int64_t>(n_i, 1), 1024);
