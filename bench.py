@@ -166,12 +166,18 @@ def cpu_baseline(wl, target_seconds: float = 12.0, steps: int = 1, min_rows: int
     s = wl.state
     xp, vp = oracle.predict_state(s)
     cores = oracle.num_threads()
-    rows = min(wl.n_i, max(cores, 16))
-    t0 = time.perf_counter()
-    oracle.regular_force(xp, vp, s.m, wl.i_idx[:rows], wl.r_s[:rows], list_stride=2 * wl.cap)
-    dt = time.perf_counter() - t0
+    # size the sample: probe with 32 rows per thread (the oracle hands out rows 16 at a time), grow the probe until it
+    # runs for a quarter of a second, then take the rows that make target_seconds of work
+    rows = min(wl.n_i, 32 * cores)
+    while True:
+        t0 = time.perf_counter()
+        oracle.regular_force(xp, vp, s.m, wl.i_idx[:rows], wl.r_s[:rows], list_stride=2 * wl.cap)
+        dt = time.perf_counter() - t0
+        if dt >= 0.25 or rows >= wl.n_i or dt >= target_seconds / 4:
+            break
+        rows = min(wl.n_i, rows * 4)
     rate = rows * s.n / dt
-    rows = int(min(wl.n_i, max(rows, min_rows, rate * target_seconds / s.n)))
+    rows = int(min(wl.n_i, max(min_rows, rate * target_seconds / s.n)))
     rows = max(cores, rows // cores * cores)
     rows = min(rows, wl.n_i)
     times, res = [], None
@@ -184,7 +190,7 @@ def cpu_baseline(wl, target_seconds: float = 12.0, steps: int = 1, min_rows: int
                sample=f"first {rows} active rows x all {s.n} j (fp64, OpenMP, gcc -O2), {dt:.2f} s per pass")
     rep.update(cpu_description())
     if single_thread:  # one thread, fewer rows (about a second of work)
-        r1 = int(max(4, min(rows, rate / max(cores, 1) * 1.0 / s.n)))
+        r1 = int(max(4, min(rows, rate / max(cores, 1) * 1.5 / s.n)))
         oracle.set_num_threads(1)
         t0 = time.perf_counter()
         oracle.regular_force(xp, vp, s.m, wl.i_idx[:r1], wl.r_s[:r1], list_stride=2 * wl.cap)
