@@ -50,9 +50,10 @@ const char* nb_strerror(int code);
 
 /* Bytes of device workspace nb_create needs for up to n_max j-particles, active blocks of up to n_i_max rows
  * and neighbour lists of nbr_cap entries per row (1 <= nbr_cap <= 8192).  Holds the packed predicted j-records
- * (40 B per j, pair-interleaved, plus a 48 B particle-major copy for nb_irregular_force) and, for the row blocks whose j-range is split over several CTAs, 56 B of
- * partial sums per (row, j-chunk): at most 112 MB, plus ~24 B per row for list-slot counters and the row ordering.  nb_create clears the
- * counters once; every call leaves them cleared.  Returns 0 if an argument is invalid. */
+ * (40 B per j, pair-interleaved, plus a 48 B particle-major copy for nb_irregular_force / nb_regular_correct) and, for
+ * the row blocks whose j-range is split over several CTAs, 64 B of partial sums per (row, j-chunk): at
+ * most 128 MB, plus ~40 B per row for list-slot counters, the queues of the fix-up passes, the error scales and the row
+ * ordering.  nb_create clears the counters once; every call leaves them cleared.  Returns 0 if an argument is invalid. */
 size_t nb_workspace_bytes(int64_t n_max, int64_t n_i_max, int32_t nbr_cap);
 
 /* cf. GPUNB_OPEN(NTOT).  Creates a context on CUDA device `device`.
@@ -245,7 +246,7 @@ int nb_fixup_stats(nb_ctx* ctx, int64_t stats[2], void* stream);
  *   "order_rows" 1 (default): large enough blocks are processed in Morton order of the predicted positions
  *               (results go to the caller's rows all the same); 0: always in the order given; 2: always ordered
  *   "fuse_pred" 1 (default): a regular-force call that finds no prediction at t, uses the plain criterion without
- *               potential and has at most 256 rows predicts inside the force kernel instead of running
+ *               potential and has at most 128 rows predicts inside the force kernel instead of running
  *               nb_predict_j first, when n >= 262144 (every j is predicted by the CTA that uses it; the context
  *               then holds no prediction at t); 0: never; 2: also for smaller n.  Results are identical bit for bit
  *   "irr_pred"  how nb_irregular_force gets its predicted particles when the context holds no prediction at t:

@@ -269,10 +269,10 @@ __device__ __forceinline__ void append(IState& I, int32_t j, bool nb, int32_t ca
 }
 
 // PRED: the predictor fused into the kernel (north_star: "fused with the Hermite predictor of the j-particles").  Used
-// for small active blocks (N_i <= 256: one to eight row blocks), whose j-range is split over the CTAs so that every j is
+// for small active blocks (N_i <= 128: one to four row blocks), whose j-range is split over the CTAs so that every j is
 // predicted by the CTA that uses it (once per row block): each thread predicts one pair of consecutive j per tile from the
 // registered fp64 state (predict_record: the arithmetic of predict.cuh, the same records bit for bit) and writes its
-// packed record straight into the shared-memory tile -- no prediction pass (38 us at N = 2^20), no packed records in
+// packed record straight into the shared-memory tile -- no prediction pass (25 us at N = 2^20), no packed records in
 // HBM.  The CTAs resident on an SM hide each other's load latency; there is one tile stage and no bulk copy.
 template <int IPT, int WARPS, int JT, int MINB, bool VEL, bool POT, bool PRED = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB) force_kernel(ForceArgs a) {

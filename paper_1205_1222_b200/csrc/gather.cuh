@@ -22,7 +22,7 @@ struct GatherArgs {
     int32_t n_i;
     const int32_t* perm;       // logical row -> caller's row (null: identity), as in ForceArgs
     int32_t n_chunks;
-    int32_t chunk_j;           // j-particles per chunk (tiles_per_chunk * j-tile)
+    int32_t chunk_j;           // j-particles per chunk (a multiple of 4, not of the tile size)
     int32_t cap;
     const double* part_sum;    // [split rows][S][7], or [..][8] with the potential: acc, jerk (, pot), error scales (float2)
     FixupFlag fix;             // rows dominated by cancellation are queued for fixup_kernel (fixflag.cuh)

@@ -220,7 +220,11 @@ namespace {
 // ragged end, which is why several waves of short CTAs beat one wave of long ones.
 // rows split into more than kWideGatherChunks chunks are gathered by a block each, if there are few enough of them
 // that a warp per row would leave SMs idle
-constexpr int kFusePredMaxRows = 256;     // largest block that predicts inside the force kernel (measured below)
+// Largest block that predicts inside the force kernel.  Round 2, after the predictor pass got its bandwidth back (38 ->
+// 25 us at N = 2^20), pass -> fused per call with a fresh prediction, replayed from a CUDA graph: N = 2^20: 32 rows 82 -> 68 us,
+// 64 rows 117 -> 106, 128 rows 190 -> 184, 256 rows 338 -> 346; N = 524288: 47 -> 43, 64 -> 61, 101 -> 101, 176 -> 182;
+// N = 262144: 33 -> 31, 42 -> 39, 60 -> 59, 98 -> 100.
+constexpr int kFusePredMaxRows = 128;
 constexpr int64_t kFusePredMinN = 262144;  // smallest n for which a one-row-block call predicts inside the force kernel
 constexpr int kOrderMinRows = 256;  // smaller active blocks are processed in the order given
 constexpr int kWideGatherChunks = 64;
@@ -609,7 +613,7 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int launches = 0;
     const bool stale = !c->predicted || c->t_pred != t;
-    // A small block (<= 256 rows) with the plain criterion predicts inside the force kernel: its j-range is split over
+    // A small block (<= 128 rows) with the plain criterion predicts inside the force kernel: its j-range is split over
     // the CTAs, so every j is predicted by the CTA that uses it (force.cuh, PRED).
     bool fuse_pred = false;
     // It pays when the prediction pass is long: measured at N = 2^20, N_i = 32: 94.8 -> 73.4 us per call (the pass costs
@@ -627,9 +631,8 @@ int nb_regular_force_ex(nb_ctx* c, int32_t n_i, const int32_t* i_idx, const doub
         const Plan p0 = make_plan(&m0, n_i, c->opt_i_block, c->opt_j_split);
         // one row block: every j predicted once.  A few row blocks: each predicts its j again, ~3 % more instructions
         // per block and 112 B/j of HBM reads that hide under the pair arithmetic, against a 38 us pass that nothing
-        // overlaps.  Measured at N = 2^20, fresh prediction per call, pass -> fused: N_i = 128: 201 -> 179 us, 256: 345 ->
-        // 337 us, 512: 606 -> 609 us: it pays up to 256 rows.  The row ordering then predicts its rows' positions itself
-        // (order.cuh, from_raw).
+        // overlaps.  It pays up to 128 rows (kFusePredMaxRows).  The row ordering, if forced, then predicts its rows'
+        // positions itself (order.cuh, from_raw).
         fuse_pred = n_i <= kFusePredMaxRows && p0.shape >= 1 && p0.shape <= 3;
     }
     if (stale && !fuse_pred) {  // the fused call: S1 first, same stream

@@ -3,7 +3,7 @@
 The paper splits the regular force over its two GPUs ("the j-particles are split ... partial
 forces and partial neighbour lists", regular-force time 45 -> 23 s).  On one NVSwitch domain the
 other axis is the natural one: the ROWS (active particles) are independent units, so every rank holds the whole
-j-set, predicts it itself (38 us at N = 2^20: cheaper than receiving it) and evaluates a contiguous slice of the
+j-set, predicts it itself (25 us at N = 2^20: cheaper than receiving it) and evaluates a contiguous slice of the
 active block.  The slices' outputs are disjoint rows of the result: the force path has NO collective.  What a host
 integrator may want afterwards -- every rank seeing all rows' acc / jerk / counts -- is one all-gather of 52 B per
 row (allgather_rows below), outside the force path.

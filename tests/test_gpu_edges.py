@@ -394,16 +394,17 @@ def test_row_ordering_paths(oracle, n_i):
     parity.check_overflow_flag(g, wl.cap)
 
 
-@pytest.mark.parametrize("n,n_i", [(5001, 1), (5001, 32), (70001, 64), (70001, 100), (30000, 128), (30000, 256), (30000, 257),
-                                  (300001, 100), (900001, 256)])
+@pytest.mark.parametrize("n,n_i", [(5001, 1), (5001, 32), (70001, 64), (70001, 100), (30000, 128), (30000, 129), (30000, 256),
+                                  (300001, 100), (900001, 128)])
 def test_prediction_fused_into_the_force_kernel_gives_the_same_bits(oracle, n, n_i):
-    """A small block (<= 256 rows) predicts inside force_kernel (PRED variant) instead of running the predictor
+    """A small block (<= 128 rows) predicts inside force_kernel (PRED variant) instead of running the predictor
     first: same records, same pair arithmetic, same row order, identical outputs; checked against the path with the
-    predictor pass (option fuse_pred = 0) bit for bit, and against the oracle as usual.  257 rows keep the pass.
-    (900001, 256) is long enough for the row ordering, which then predicts its rows' positions itself."""
+    predictor pass (option fuse_pred = 0) bit for bit, and against the oracle as usual.  129 and 256 rows keep the pass.
+    (900001, 128) runs with the row ordering forced, which then predicts its rows' positions itself."""
     wl = inputs.make_custom(n, n_i, 20, 64, seed_sub=7, predict=lambda s: oracle.predict_state(s)[0])
     s = wl.state
     ctx = binding.Context(s.n, max(n_i, 1), wl.cap)
+    ctx.nb_set_option("order_rows", 2 if n == 900001 else 1)
     res = {}
     big = n >= 262144                             # there the default setting (1) fuses by itself
     # Both paths on the SAME launch plan: the fused-prediction kernels hold 24 warps per SM against 28, so the planner
@@ -420,7 +421,7 @@ def test_prediction_fused_into_the_force_kernel_gives_the_same_bits(oracle, n, n
     (g1, i1), (g0, i0) = res[2], res[0]
     assert i1["j_chunks"] == i0["j_chunks"] and i1["rows_per_cta"] == i0["rows_per_cta"]
     # predictor, [row ordering: one kernel up to 8192 rows, when the call is long enough], force, gather
-    assert i0["launches"] - i1["launches"] == (1 if n_i <= 256 else 0)
+    assert i0["launches"] - i1["launches"] == (1 if n_i <= 128 else 0)
     for k in ("acc", "jerk", "nbr_count", "n_overflow"):
         assert np.array_equal(g1[k], g0[k]), k
     for q in range(n_i):

@@ -47,7 +47,7 @@ def test_forced_on_every_row_it_is_the_fp64_sum(oracle, n_i, opts):
 
 
 def test_forced_with_velocity_criterion_potential_and_fused_prediction(oracle):
-    wl = _wl(oracle, 5003, 130, 20, 64)
+    wl = _wl(oracle, 5003, 100, 20, 64)
     xp, vp = oracle.predict_state(wl.state)
     dtr = (wl.state.t - wl.state.t0[wl.i_idx]) * 4.0
     g, info = run_gpu(wl, options=ALL_ROWS, dtr=dtr, want_pot=True)
