@@ -39,6 +39,7 @@ extern "C" {
 #define NB_E_STATE (-2) /* call out of order: force/predict before nb_set_j, get_predicted before predict */
 #define NB_E_NOMEM (-3) /* workspace too small, or a device allocation failed                            */
 #define NB_E_CUDA (-4)  /* CUDA runtime / launch error                                                     */
+#define NB_E_LIMIT (-5) /* size beyond the fixed limits of nb_regular_force_static                         */
 
 typedef struct nb_ctx nb_ctx;
 
@@ -239,6 +240,27 @@ int nb_regular_force_host_csr(nb_ctx* ctx, int64_t n, const double* x0, const do
  *                 Synchronises `stream`. */
 int nb_get_error_scale(nb_ctx* ctx, int32_t n_i, float* escale, void* stream);
 int nb_fixup_stats(nb_ctx* ctx, int64_t stats[2], void* stream);
+
+/* The regular-force call (step (vi), eq. (9)-(11), after predicting all n particles to t, step (iii),
+ * PAPER.md:93) for callers that MUST NOT ALLOCATE: code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc.  No context and no workspace: all scratch (packed predicted records, partial sums of j-split rows,
+ * counters and queues) lives in one file-scope device array of 8 MiB inside the library, which every GPU that loads the
+ * library holds until the process exits.  The call makes no cudaMalloc / cudaFree and calls no allocating routine.
+ *   LIMITS: n <= 65536, n_i <= 4096, nbr_cap <= 512 (nb_static_limits reports them: {n, n_i, nbr_cap, scratch bytes});
+ *           beyond them the call returns NB_E_LIMIT and enqueues nothing -- use nb_create + nb_regular_force instead.
+ *   device: CUDA device ordinal; the array of THAT device is used (set up at the first call for the device: symbol
+ *           address, kernel attributes -- make that first call outside a graph capture).
+ *   x0, v0, a0, j0: dev double[n][3]; m, t0: dev double[n]  (16-byte aligned), as nb_set_j
+ *   i_idx, r_s, acc, jerk, nbr_count, nbr_list ([n_i][nbr_cap]), n_overflow: dev, as nb_regular_force
+ * Same kernels, same arithmetic, same fp64 fix-up pass as nb_regular_force (plain criterion, rows in the order given);
+ * only the launch plan may differ (fewer j-chunks fit the array), i.e. the sums agree to rounding, lists and counts
+ * exactly.  ALL CALLS ON A DEVICE SHARE THE ARRAY, which keeps the last call's contents: the call clears what must start
+ * at zero, on `stream`; calls that overlap on the GPU (two streams, two threads) race -- keep them on one stream. */
+int nb_regular_force_static(int device, int64_t n, const double* x0, const double* v0, const double* a0,
+                            const double* j0, const double* m, const double* t0, int32_t n_i, const int32_t* i_idx,
+                            const double* r_s, double t, int32_t nbr_cap, double* acc, double* jerk,
+                            int32_t* nbr_count, int32_t* nbr_list, int32_t* n_overflow, void* stream);
+int nb_static_limits(int64_t limits[4]);
 
 /* Tuning knobs (tests and benchmarks).  key:
  *   "j_split"   force the number of j-chunks per row for ALL row blocks (0 = automatic; 1 = never split)

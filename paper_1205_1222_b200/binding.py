@@ -55,6 +55,9 @@ def load(build_if_missing: bool = True):
     lib.nb_regular_force_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp]
     lib.nb_regular_force_host_csr.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, dbl, vp, vp, vp, vp, vp, i64, vp]
     lib.nb_set_option.argtypes = [vp, ctypes.c_char_p, i64]
+    lib.nb_regular_force_static.argtypes = [ctypes.c_int, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, dbl, i32, vp, vp, vp, vp,
+                                            vp, vp]
+    lib.nb_static_limits.argtypes = [ctypes.POINTER(i64)]
     lib.nb_get_error_scale.argtypes = [vp, i32, vp, vp]
     lib.nb_fixup_stats.argtypes = [vp, ctypes.POINTER(i64), vp]
     lib.nb_last_launch_info.argtypes = [vp, ctypes.POINTER(i64)]
@@ -106,6 +109,28 @@ def nb_plan(n: int, n_i: int, num_sms: int = 148, ctas_per_sm=(3, 6, 12, 24, 1),
     _check(load().nb_plan(int(n), int(n_i), int(num_sms), occ, int(i_block), int(j_split), arr))
     keys = tuple("chunk_j" if k == "launches" else k for k in _INFO_KEYS)
     return dict(zip(keys, [int(v) for v in arr]))
+
+
+def nb_static_limits() -> dict:
+    """Limits of nb_regular_force_static: n, n_i, nbr_cap, and the bytes of its file-scope device scratch array."""
+    arr = (ctypes.c_int64 * 4)()
+    _check(load().nb_static_limits(arr))
+    return dict(n=int(arr[0]), n_i=int(arr[1]), nbr_cap=int(arr[2]), scratch_bytes=int(arr[3]))
+
+
+def nb_regular_force_static(x0, v0, a0, j0, m, t0, i_idx, r_s, t: float, out: dict, device: int = 0, stream=None):
+    """nb_regular_force_static: the allocation-free call (no context, no workspace; scratch in a fixed device array of the
+    library).  All tensors on cuda:`device`; `out` holds acc, jerk, nbr_count, nbr_list [n_i][nbr_cap], n_overflow."""
+    f64 = torch.float64
+    n, n_i = int(x0.shape[0]), int(i_idx.shape[0])
+    cap = int(out["nbr_list"].shape[1]) if out["nbr_list"].dim() == 2 else 1
+    _check(load().nb_regular_force_static(
+        int(device), n, _dev(x0, f64, "x0"), _dev(v0, f64, "v0"), _dev(a0, f64, "a0"), _dev(j0, f64, "j0"),
+        _dev(m, f64, "m"), _dev(t0, f64, "t0"), n_i, _dev(i_idx, torch.int32, "i_idx"), _dev(r_s, f64, "r_s"), float(t),
+        cap, _dev(out["acc"], f64, "acc"), _dev(out["jerk"], f64, "jerk"),
+        _dev(out["nbr_count"], torch.int32, "nbr_count"), _dev(out["nbr_list"], torch.int32, "nbr_list"),
+        _dev(out["n_overflow"], torch.int32, "n_overflow"), _stream_ptr(stream)))
+    return out
 
 
 class Context:

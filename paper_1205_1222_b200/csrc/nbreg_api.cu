@@ -454,6 +454,9 @@ const char* nb_strerror(int code) {
         case NB_E_STATE: return "call out of order (no j-state registered / nothing predicted yet)";
         case NB_E_NOMEM: return "workspace too small or device allocation failed";
         case NB_E_CUDA: return g_errbuf[0] ? g_errbuf : "CUDA error";
+        case NB_E_LIMIT:
+            return "size beyond the limits of the static-scratch entry point nb_regular_force_static "
+                   "(n <= 65536, n_i <= 4096, nbr_cap <= 512): use nb_create + nb_regular_force";
         default: return "unknown error code";
     }
 }
@@ -1195,3 +1198,142 @@ int nb_last_launch_info(const nb_ctx* c, int64_t info[8]) {
 }
 
 }  // extern "C"
+
+// =====================================================================================================================
+// nb_regular_force_static: the regular-force call for callers that must not allocate (code under CUDA graph capture,
+// tight serving loops, harnesses that forbid cudaMalloc).  No context, no workspace argument, no cudaMalloc / cudaFree /
+// allocating library routine anywhere on its path: ALL scratch of the call -- the packed predicted j-records, the
+// partial sums of the j-split rows, the list-slot counters, the queues and control words of the gather and fix-up
+// kernels -- lives in ONE file-scope device array of kStaticScratchBytes = 8 MiB, which every GPU that loads the library
+// holds until the process exits.  Hence the limits: n <= 65536, n_i <= 4096, nbr_cap <= 512.
+//
+// g_static_scratch below is, in HOST code, a host-side stand-in for the device array, not a device address: a kernel
+// handed that name would fault (or, where the GPU can reach host memory, silently use the wrong memory).  The device
+// address is obtained once per device, with that device current, by cudaGetSymbolAddress, and it is that pointer the
+// kernels get.  The same kernels as nb_regular_force run (predict_kernel, force_kernel, the gather kernel, fixup_kernel),
+// planned with the smaller number of (row, j-chunk) slots the array has room for.
+//
+// Every call on a device shares the array, and it keeps the last call's contents: the words that must start at zero
+// (slot counters, tickets, queue lengths) are cleared at the start of every call, on the caller's stream.  Calls that
+// overlap on the GPU (two streams, two host threads) RACE on the array: keep the calls of one device on one stream.
+// The host-side set-up of a device (symbol address, kernel attributes, occupancy) happens in the first call for that
+// device: make that call outside a graph capture.
+namespace {
+
+constexpr size_t kStaticScratchBytes = 8u << 20;
+constexpr int64_t kStaticMaxN = 65536, kStaticMaxNi = 4096;
+constexpr int32_t kStaticMaxCap = 512;
+constexpr int64_t kStaticRowChunkSlots = 65536;  // (row, j-chunk) partial sums of 64 B: 4 MiB of the array
+constexpr int kStaticMaxDevices = 64;
+
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+struct StaticSlot {
+    bool ready = false;
+    nb_ctx ctx;  // a context object in static storage (never nb_create'd, never destroyed); ctx.ws = the symbol's address
+};
+StaticSlot g_static[kStaticMaxDevices];
+
+// The workspace layout of layout() (above) cut down to what the static call uses: no particle-major copy (no gathering
+// consumer), no row-ordering buffers (blocks this small are processed in the order given), kStaticRowChunkSlots slots.
+WorkspaceLayout static_layout() {
+    WorkspaceLayout w{};
+    const int64_t n_pad = round_up(kStaticMaxN, kJPad);
+    w.row_chunk_limit = kStaticRowChunkSlots;
+    size_t off = 0;
+    auto place = [&](size_t bytes, size_t& o, size_t& b) {
+        o = off;
+        b = bytes;
+        off += (size_t)round_up((int64_t)bytes, 256);
+    };
+    place((size_t)n_pad * kBytesPerJ, w.packed_off, w.packed_bytes);
+    place(std::max((size_t)w.row_chunk_limit * 8 * sizeof(double),
+                   ((size_t)kFixMaxGrid * kFixWarps + (size_t)kStaticMaxNi + kFixWarps) * 6 * sizeof(double)),
+          w.psum_off, w.psum_bytes);
+    place((size_t)(n_pad / kJPad) * sizeof(float), w.vmax_off, w.vmax_bytes);
+    place((size_t)(kStaticMaxNi + 1) * sizeof(int32_t), w.fixrow_off, w.fixrow_bytes);
+    place((size_t)(kStaticMaxNi + 1) * sizeof(float2), w.escale_off, w.escale_bytes);
+    place((size_t)(kStaticMaxNi + 1) * sizeof(int32_t), w.ovfrow_off, w.ovfrow_bytes);
+    // from here on: zero at the start of every call
+    place((size_t)(kStaticMaxNi + 512) * sizeof(int32_t), w.slot_off, w.slot_bytes);
+    place((size_t)(kStaticMaxNi / kFixWarps + 34) * sizeof(int32_t), w.ftick_off, w.ftick_bytes);
+    place(128, w.ctl_off, w.ctl_bytes);
+    w.total = off;
+    return w;
+}
+
+// Once per device, with that device current: the device address of the scratch array, the kernel attributes and
+// occupancy figures nb_create would have set up.  Nothing here allocates.
+int static_setup(int device, StaticSlot** out) {
+    if (device < 0 || device >= kStaticMaxDevices) return NB_E_INVAL;
+    StaticSlot& sl = g_static[device];
+    *out = &sl;
+    if (sl.ready) return NB_OK;
+    int ndev = 0;
+    NB_CUDA(cudaGetDeviceCount(&ndev));
+    if (device >= ndev) return NB_E_INVAL;
+    NB_CUDA(cudaSetDevice(device));
+    nb_ctx& c = sl.ctx;
+    c.lay = static_layout();
+    if (c.lay.total > kStaticScratchBytes) return NB_E_NOMEM;  // (cannot happen: the constants above are sized to fit)
+    void* dev_ptr = nullptr;
+    NB_CUDA(cudaGetSymbolAddress(&dev_ptr, g_static_scratch));  // NOT &g_static_scratch: that is a host address
+    if (!dev_ptr || (reinterpret_cast<uintptr_t>(dev_ptr) & 255u)) {
+        snprintf(g_errbuf, sizeof(g_errbuf), "cudaGetSymbolAddress(g_static_scratch) gave an unusable address");
+        return NB_E_CUDA;
+    }
+    c.ws = static_cast<unsigned char*>(dev_ptr);
+    c.ws_owned = false;
+    c.device = device;
+    NB_CUDA(cudaDeviceGetAttribute(&c.num_sms, cudaDevAttrMultiProcessorCount, device));
+    // function attributes are per process (nb_create sets the same ones)
+    NB_CUDA(cudaFuncSetAttribute(reduce_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)((size_t)kGatherWarps * (kMaxNbrCap + kMaxChunks) * sizeof(int32_t))));
+    NB_CUDA(cudaFuncSetAttribute(reduce_gather_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)((size_t)kMaxNbrCap * sizeof(int32_t))));
+    for (int k = 0; k < kNumShapes; ++k) {  // plain criterion, no potential: variant 0
+        const int rc = force_dispatch(0, k, &c.ctas_per_sm[0][k], nullptr, nullptr, nullptr);
+        if (rc != NB_OK) return rc;
+    }
+    c.n_max = kStaticMaxN;
+    c.n_i_max = kStaticMaxNi;
+    c.cap = kStaticMaxCap;
+    c.opt_order_rows = 0;   // no ordering buffers in the array
+    c.opt_fuse_pred = 0;    // always the predictor pass into the array's packed records
+    sl.ready = true;
+    return NB_OK;
+}
+
+}  // namespace
+
+extern "C" int nb_regular_force_static(int device, int64_t n, const double* x0, const double* v0, const double* a0,
+                                       const double* j0, const double* m, const double* t0, int32_t n_i,
+                                       const int32_t* i_idx, const double* r_s, double t, int32_t nbr_cap, double* acc,
+                                       double* jerk, int32_t* nbr_count, int32_t* nbr_list, int32_t* n_overflow,
+                                       void* stream) {
+    if (n < 1 || n_i < 0 || nbr_cap < 1 || !n_overflow) return NB_E_INVAL;
+    if (n > kStaticMaxN || n_i > kStaticMaxNi || nbr_cap > kStaticMaxCap) return NB_E_LIMIT;
+    StaticSlot* sl = nullptr;
+    int rc = static_setup(device, &sl);
+    if (rc != NB_OK) return rc;
+    nb_ctx* c = &sl->ctx;
+    NB_CUDA(cudaSetDevice(device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    // the array keeps the last call's contents: what must start at zero is cleared here, on the caller's stream
+    NB_CUDA(cudaMemsetAsync(c->ws + c->lay.slot_off, 0, c->lay.ctl_off + c->lay.ctl_bytes - c->lay.slot_off, st));
+    c->cap = nbr_cap;
+    rc = nb_set_j(c, n, x0, v0, a0, j0, m, t0);  // registers the pointers; the prediction is now stale ...
+    if (rc != NB_OK) return rc;
+    // ... so this predicts all n particles into the array first, then runs force, gather and fix-up kernels
+    return nb_regular_force_ex(c, n_i, i_idx, r_s, nullptr, t, acc, jerk, nullptr, nbr_count, nbr_list, n_overflow,
+                               stream);
+}
+
+extern "C" int nb_static_limits(int64_t limits[4]) {
+    if (!limits) return NB_E_INVAL;
+    limits[0] = kStaticMaxN;
+    limits[1] = kStaticMaxNi;
+    limits[2] = kStaticMaxCap;
+    limits[3] = (int64_t)kStaticScratchBytes;
+    return NB_OK;
+}
