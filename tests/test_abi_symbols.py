@@ -38,6 +38,20 @@ def test_host_side_logic_without_gpu():
     assert lib.nb_set_option(None, b"j_split", 1) == -1
 
 
+def test_static_entry_point_limits_are_checked_before_any_cuda_call():
+    """nb_regular_force_static (scratch in a fixed 8 MiB device array of the library) rejects sizes beyond its limits with
+    NB_E_LIMIT and a text that names the entry point -- on a box without a GPU too."""
+    lib = binding.load()
+    assert binding.nb_static_limits() == dict(n=65536, n_i=4096, nbr_cap=512, scratch_bytes=8 << 20)
+    one = ctypes.c_int32(0)
+    p = ctypes.cast(ctypes.pointer(one), ctypes.c_void_p)
+    call = lambda n, n_i, cap: lib.nb_regular_force_static(0, n, p, p, p, p, p, p, n_i, p, p, 1.0, cap, p, p, p, p, p, None)
+    for args in ((65537, 1, 8), (100, 4097, 8), (100, 1, 513)):
+        rc = call(*args)
+        assert rc == -5 and b"nb_regular_force_static" in lib.nb_strerror(rc)
+    assert call(0, 1, 8) == -1 and call(100, -1, 8) == -1 and call(100, 1, 0) == -1
+
+
 def test_binding_fails_loudly_without_cuda():
     import pytest
     import torch

@@ -438,3 +438,22 @@ def test_prediction_fused_into_the_force_kernel_gives_the_same_bits(oracle, n, n
     g2, i2 = run_gpu(wl, ctx=ctx, dtr=np.zeros(n_i))
     assert i2["launches"] == i0["launches"] and np.allclose(g2["acc"], g1["acc"], rtol=1e-5, atol=0)
     ctx.close()
+
+
+def test_launch_and_copy_options_do_not_change_the_bits(oracle):
+    """Options that only change HOW the kernels are launched or what else the predictor writes: "pdl" (programmatic
+    dependent launch along the kernel chain) and "gather_copy" (the particle-major copy of the records, written for the
+    gathering kernels): identical outputs bit for bit, on a j-split block with the fix-up pass at work."""
+    wl = _wl(oracle, 7001, 900, 20, 64, masses="salpeter")
+    ref, info = run_gpu(wl)
+    assert info["j_chunks"] > 1
+    try:
+        for opts in ({"pdl": 0}, {"pdl": 1, "gather_copy": 1}, {"pdl": 0, "gather_copy": 1}):
+            g, _ = run_gpu(wl, options=opts)
+            for k in ("acc", "jerk", "nbr_count", "nbr_list", "n_overflow"):
+                assert np.array_equal(g[k], ref[k]), (opts, k)
+    finally:  # "pdl" is process-wide: leave it on for the tests that follow
+        ctx = binding.Context(16, 16, 8)
+        ctx.nb_set_option("pdl", 1)
+        ctx.close()
+    _full_check(oracle, wl, ref)
