@@ -124,6 +124,7 @@ __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
             I.dtr = VEL ? __double2float_rn(a.dtr[orow]) : 0.f;
         }
         double s[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        const double h2_near = 1.01 * (double)I.h2;
         const int32_t t_end = min((c + 1) * tpc, n_tiles);
         for (int32_t t = c * tpc; t < t_end; ++t) {
             __syncthreads();  // the previous tile has been read by every warp
@@ -152,22 +153,26 @@ __global__ void __launch_bounds__(kFixThreads) fixup_kernel(FixupArgs a) {
             for (int32_t jj = sub * 32 + lane; jj < jn; jj += 32 * nsub) {
                 const int32_t j = t * kFixThreads + jj;
                 if (j == i) continue;
-                // the neighbour test of force_kernel's near path, on the same fp32 words (both halves hold j)
-                const float4 q0 = make_float4(sh[0][jj], sh[0][jj], sh[1][jj], sh[1][jj]);
-                const float4 q1 = make_float4(sh[2][jj], sh[2][jj], 0.f, 0.f);
-                const float4 q2 = make_float4(sw[0][jj], sw[0][jj], sw[1][jj], sw[1][jj]);
-                const float2 vz = make_float2(sw[2][jj], sw[2][jj]);
-                const float2 xl = make_float2(sl[0][jj], sl[0][jj]);
-                const float4 q4 = make_float4(sl[1][jj], sl[1][jj], sl[2][jj], sl[2][jj]);
-                PairGeom gm;
-                geom_hi(q0, q1, I, gm);
-                geom_lo(xl, q4, I, gm);
-                const float2 rm = VEL ? rmin2_velocity(q2, vz, I, gm) : gm.r2;
-                if (rm.x < I.h2) continue;  // neighbour: listed by force_kernel, not summed
-                // eq. (9), (10) in fp64
                 const double Rx = sx[0][jj] - xi[0], Ry = sx[1][jj] - xi[1], Rz = sx[2][jj] - xi[2];
-                const double Vx = sv[0][jj] - vi[0], Vy = sv[1][jj] - vi[1], Vz = sv[2][jj] - vi[2];
                 const double r2 = Rx * Rx + Ry * Ry + Rz * Rz;
+                // The neighbour test of force_kernel's near path, on the same fp32 words (both halves hold j).  With the
+                // plain criterion it is needed only close to r_s: the fp32 r^2 of the two-float difference is within
+                // ~1e-6 of the fp64 one, so a pair with r^2 >= 1.01 r_s^2 cannot be a neighbour by it.
+                if (VEL || r2 < h2_near) {
+                    const float4 q0 = make_float4(sh[0][jj], sh[0][jj], sh[1][jj], sh[1][jj]);
+                    const float4 q1 = make_float4(sh[2][jj], sh[2][jj], 0.f, 0.f);
+                    const float4 q2 = make_float4(sw[0][jj], sw[0][jj], sw[1][jj], sw[1][jj]);
+                    const float2 vz = make_float2(sw[2][jj], sw[2][jj]);
+                    const float2 xl = make_float2(sl[0][jj], sl[0][jj]);
+                    const float4 q4 = make_float4(sl[1][jj], sl[1][jj], sl[2][jj], sl[2][jj]);
+                    PairGeom gm;
+                    geom_hi(q0, q1, I, gm);
+                    geom_lo(xl, q4, I, gm);
+                    const float2 rm = VEL ? rmin2_velocity(q2, vz, I, gm) : gm.r2;
+                    if (rm.x < I.h2) continue;  // neighbour: listed by force_kernel, not summed
+                }
+                // eq. (9), (10) in fp64
+                const double Vx = sv[0][jj] - vi[0], Vy = sv[1][jj] - vi[1], Vz = sv[2][jj] - vi[2];
                 if (r2 == 0.0) continue;  // coincident (reading R4)
                 const double ri = rsqrt(r2), ri2 = ri * ri;
                 const double mri3 = sm[jj] * ri * ri2;
