@@ -9,11 +9,13 @@
 // neighbour, so the result stays the sum over exactly the complement of the emitted list.  (A pair force_kernel took
 // on its far path is never a neighbour by that test either: the far threshold carries a 2^-10 margin, force.cuh.)
 //
-// Mapping: the queued rows are taken R at a time (R = 8, 4, 2 or 1: few rows -> all eight warps of a CTA on one row);
-// a work item is (group of R rows, j-chunk).  The 256 threads of a CTA predict a tile of 256 j straight from the
-// registered fp64 state into shared memory (the Horner form of predict.cuh; fp64 x_p, v_p, m and the fp32 record the
-// neighbour test needs), then every warp runs its row over its share of the tile, lanes striding over j.  Lane sums are fp64, reduced by a fixed xor-shuffle tree; the chunks of a
-// row are added in a fixed order by the CTA that finishes last (atomic ticket): deterministic for a given device.
+// Mapping: the queued rows are taken R at a time (R = 8, or 4, 2, 1 when fewer than five rows are queued: the idle
+// warps of a CTA then share a row); a work item is (group of R rows, j-chunk), and there are as many chunks as fill one
+// wave of the grid.  The 256 threads of a CTA predict a tile of 256 j straight from the registered fp64 state into
+// shared memory (the Horner form of predict.cuh; fp64 x_p, v_p, m and the fp32 record the neighbour test needs), then
+// every warp runs its row over its share of the tile, lanes striding over j.  Lane sums are fp64, reduced by a fixed
+// xor-shuffle tree; the warps that share a row are added in order, the chunks of a row in a fixed order by the CTA that
+// finishes last (atomic ticket): deterministic for a given device.
 // The pass always runs (one launch); with nothing queued every CTA returns at once.
 #pragma once
 #include "fixflag.cuh"
